@@ -1,0 +1,119 @@
+/* spiir.h -- C ABI of the B200-native SPIIR template-bank filter.
+ *
+ * Operation (BASELINE.json:north_star; section 3.1 "a parallel bank of single pole IIR
+ * filters", section 3.3 "parameter array and the detection data within given time window
+ * ... output data of each filter which is the input data in the next iteration", L329/L339 "The SNR of
+ * one template needs the outputs of all its filters ... sum all the output"):
+ *
+ *     y_{t,k}[n] = a1_{t,k} * y_{t,k}[n-1] + b0_{t,k} * x[n - d_{t,k}]
+ *     SNR_t[n]   = sum_k y_{t,k}[n]
+ *
+ * a1, b0 complex, d integer >= 0, x real (whitened strain).  All arithmetic is FP32 on the GPU.
+ * Semantics fixed at this boundary: zero initial state y[-1] = 0; zero
+ * pre-history x[m<0] = 0; d = 0 is the current sample; the sample index is global across calls; the
+ * output is the plain sum (no normalisation); the order of a template's filters does not matter
+ * (up to rounding).  The summation order is fixed by the bank layout, so results are bitwise
+ * reproducible from run to run and independent of a template's position in the bank.
+ *
+ * Every step of the path runs in the library's own CUDA kernels (sm_100a).  There is no CPU fallback:
+ * without a CUDA device every call that needs one fails with SPIIR_ECUDA.
+ *
+ * Threading: a handle is not thread-safe; distinct handles are.  Work is enqueued on the caller's
+ * stream and is ordered with respect to it; calls return without synchronising the host unless noted.
+ */
+#ifndef SPIIR_H
+#define SPIIR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spiir_bank spiir_bank; /* opaque; owns device coefficients, filter state, input history */
+
+enum {
+    SPIIR_OK = 0,
+    SPIIR_EINVAL = -1, /* bad argument (null, negative, inconsistent sizes, non-finite, |a1| >= 1) */
+    SPIIR_ENOMEM = -2, /* host or device allocation failed */
+    SPIIR_ECUDA = -3,  /* CUDA runtime / launch error, or no usable device */
+    SPIIR_ESTATE = -4  /* handle unusable (a previous call failed part-way) */
+};
+
+/* Kernel path used by spiir_filter (north_star subsystems (3) and (4)). */
+enum {
+    SPIIR_PATH_AUTO = 0,       /* choose per call from bank size and chunk length */
+    SPIIR_PATH_THROUGHPUT = 1, /* filters across lanes, sequential in time, smem-staged window */
+    SPIIR_PATH_SCAN = 2,       /* time-parallel: segments per filter + linear-recurrence carry scan */
+    SPIIR_PATH_STREAM = 3      /* tiny chunks, many filters: one pass over coefficients+state (HBM bound) */
+};
+
+typedef struct spiir_options {
+    int32_t struct_size;        /* = sizeof(spiir_options); lets the struct grow compatibly */
+    int32_t path;               /* SPIIR_PATH_*; default AUTO */
+    int32_t filters_per_thread; /* 0 = choose; else 2, 4, 8 or 16 (register blocking of the throughput kernel) */
+    int32_t scan_segments;      /* 0 = choose; else time segments per call for SPIIR_PATH_SCAN */
+    int32_t reserved[4];        /* must be 0 */
+} spiir_options;
+
+/* Build a bank.  All pointers are HOST pointers; the arrays are copied, the caller keeps ownership.
+ *   n_templates      T >= 1
+ *   filter_offsets   [T+1] CSR offsets into the filter arrays, offsets[0] = 0, strictly increasing
+ *                    (every template has >= 1 filter); K = offsets[T]
+ *   a1, b0           [2K] float32, (re, im) interleaved = complex64; |a1| < 1 and everything finite
+ *   delays           [K] int32, d >= 0
+ *   device           CUDA device ordinal
+ *   opt              nullable (defaults)
+ * The bank lays the filters out on the device in structure-of-arrays form, each template's filters
+ * sorted by delay, dealt to lanes so that a warp's shared-memory reads of x[n-d] avoid bank
+ * conflicts, and padded with null filters (a1 = b0 = 0) to the kernel's tile size (north_star
+ * subsystem (1); "aligned and continuous").  State and history start at zero.
+ * Synchronises the host with the device.  On error *out is NULL. */
+int spiir_bank_create(spiir_bank **out, int32_t n_templates, const int64_t *filter_offsets,
+                      const float *a1, const float *b0, const int32_t *delays, int32_t device,
+                      const spiir_options *opt);
+
+/* Filter the next n samples of strain.
+ *   x_dev     DEVICE pointer, [n] float32, caller-owned
+ *   snr_dev   DEVICE pointer, complex64 as (re, im) float32 pairs; row t starts at snr_dev + 2*t*ld;
+ *             exactly SNR[t][0..n) is written for every template t, nothing else is touched
+ *   ld        row stride in complex elements, ld >= n (lets chunked calls fill columns of one [T][N] buffer)
+ *   stream    cudaStream_t (NULL = legacy default stream)
+ * n = 0 is a no-op.  Any n >= 1 and any sequence of chunk sizes is valid, including n smaller than the
+ * largest delay.  Carries filter state y and the last max_delay input samples to the next call.
+ * Enqueues on the stream and returns; x_dev and snr_dev must stay valid until the stream reaches
+ * that point.  SPIIR_EINVAL on null pointers, n < 0 or ld < n; SPIIR_ECUDA on launch failure. */
+int spiir_filter(spiir_bank *bank, const float *x_dev, int64_t n, float *snr_dev, int64_t ld,
+                 void *stream);
+
+/* Same operation with HOST buffers (the end-to-end entry): copies x to the device, filters, copies
+ * SNR[t][0..n) back into snr_host (row stride ld), overlapping copies and kernels internally.
+ * Buffers may be pageable or pinned.  Returns after the results are in snr_host. */
+int spiir_filter_host(spiir_bank *bank, const float *x_host, int64_t n, float *snr_host, int64_t ld);
+
+/* Zero the filter state and the input history (a cold bank again); enqueued on the stream. */
+int spiir_bank_reset(spiir_bank *bank, void *stream);
+
+/* Sizes.  Return -1 for a null handle. */
+int64_t spiir_bank_num_templates(const spiir_bank *bank);
+int64_t spiir_bank_num_filters(const spiir_bank *bank); /* real filters K, padding excluded */
+int64_t spiir_bank_max_delay(const spiir_bank *bank);   /* D = max_k d_k = length of the carried history */
+
+/* Checkpoint / resume.  y_dev: DEVICE [2K] float32 (re, im) in the CALLER's filter order;
+ * hist_dev: DEVICE [D] float32, hist[j] = x[n_done - D + j] (oldest first).  Either may be NULL to skip it. */
+int spiir_bank_get_state(spiir_bank *bank, float *y_dev, float *hist_dev, void *stream);
+int spiir_bank_set_state(spiir_bank *bank, const float *y_dev, const float *hist_dev, void *stream);
+
+/* Free everything the bank owns (synchronises the device).  NULL is a no-op. */
+int spiir_bank_destroy(spiir_bank *bank);
+
+/* Introspection. */
+const char *spiir_last_error(void);      /* thread-local message of the last failing call */
+int64_t spiir_kernel_launches(void);     /* kernels this library has launched in this process */
+int32_t spiir_bank_last_path(const spiir_bank *bank); /* SPIIR_PATH_* used by the last spiir_filter */
+int32_t spiir_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPIIR_H */

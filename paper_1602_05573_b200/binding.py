@@ -1,0 +1,235 @@
+"""ctypes binding of include/spiir.h -- argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libspiir_b200.so"
+_lib = None
+
+PATH_AUTO, PATH_THROUGHPUT, PATH_SCAN, PATH_STREAM = 0, 1, 2, 3
+
+EXPORTS = ["spiir_bank_create", "spiir_filter", "spiir_filter_host", "spiir_bank_reset",
+           "spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay",
+           "spiir_bank_get_state", "spiir_bank_set_state", "spiir_bank_destroy", "spiir_last_error",
+           "spiir_kernel_launches", "spiir_bank_last_path", "spiir_version"]
+
+
+class SpiirError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"spiir error {code}: {msg}")
+        self.code = code
+
+
+class SpiirOptions(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_int32), ("path", ctypes.c_int32),
+                ("filters_per_thread", ctypes.c_int32), ("scan_segments", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 4)]
+
+    def __init__(self, path: int = PATH_AUTO, filters_per_thread: int = 0, scan_segments: int = 0):
+        super().__init__()
+        self.struct_size = ctypes.sizeof(SpiirOptions)
+        self.path, self.filters_per_thread, self.scan_segments = path, filters_per_thread, scan_segments
+
+
+def library_path() -> Path:
+    return _LIB_PATH
+
+
+def load_library():
+    """Load libspiir_b200.so (built in-tree by ``__graft_entry__.build()``); fails loudly if missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise FileNotFoundError(f"{_LIB_PATH} is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                                "(there is no CPU fallback)")
+    lib = ctypes.CDLL(str(_LIB_PATH))
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    lib.spiir_bank_create.restype = ctypes.c_int
+    lib.spiir_bank_create.argtypes = [ctypes.POINTER(vp), i32, vp, vp, vp, vp, i32, ctypes.POINTER(SpiirOptions)]
+    lib.spiir_filter.restype = ctypes.c_int
+    lib.spiir_filter.argtypes = [vp, vp, i64, vp, i64, vp]
+    lib.spiir_filter_host.restype = ctypes.c_int
+    lib.spiir_filter_host.argtypes = [vp, vp, i64, vp, i64]
+    lib.spiir_bank_reset.restype = ctypes.c_int
+    lib.spiir_bank_reset.argtypes = [vp, vp]
+    for name in ("spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay"):
+        getattr(lib, name).restype = i64
+        getattr(lib, name).argtypes = [vp]
+    lib.spiir_bank_get_state.restype = ctypes.c_int
+    lib.spiir_bank_get_state.argtypes = [vp, vp, vp, vp]
+    lib.spiir_bank_set_state.restype = ctypes.c_int
+    lib.spiir_bank_set_state.argtypes = [vp, vp, vp, vp]
+    lib.spiir_bank_destroy.restype = ctypes.c_int
+    lib.spiir_bank_destroy.argtypes = [vp]
+    lib.spiir_last_error.restype = ctypes.c_char_p
+    lib.spiir_kernel_launches.restype = i64
+    lib.spiir_bank_last_path.restype = i32
+    lib.spiir_bank_last_path.argtypes = [vp]
+    lib.spiir_version.restype = i32
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise SpiirError(rc, load_library().spiir_last_error().decode())
+
+
+def _ptr(a: np.ndarray):
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+def _stream_handle(stream) -> ctypes.c_void_p:
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return ctypes.c_void_p(stream)
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def spiir_bank_create(filter_offsets, a1, b0, delays, device: int = 0, options: SpiirOptions | None = None):
+    """-> opaque bank handle.  Host numpy arrays: int64 [T+1], complex64 [K], complex64 [K], int32 [K]."""
+    lib = load_library()
+    off = np.ascontiguousarray(filter_offsets, dtype=np.int64)
+    a1 = np.ascontiguousarray(a1, dtype=np.complex64)
+    b0 = np.ascontiguousarray(b0, dtype=np.complex64)
+    d = np.ascontiguousarray(delays, dtype=np.int32)
+    K = int(off[-1]) if off.size else 0
+    if off.ndim != 1 or off.size < 1 or not (a1.shape == b0.shape == d.shape == (K,)):
+        raise ValueError("filter_offsets must be [T+1] and a1, b0, delays must have filter_offsets[-1] entries")
+    h = ctypes.c_void_p()
+    _check(lib.spiir_bank_create(ctypes.byref(h), off.size - 1, _ptr(off), _ptr(a1), _ptr(b0), _ptr(d),
+                                 device, ctypes.byref(options) if options is not None else None))
+    return h
+
+
+def spiir_filter(bank, x, snr, ld: int | None = None, stream=None, n: int | None = None):
+    """x: CUDA float32 tensor [n]; snr: CUDA complex64 tensor whose row t starts ``ld`` elements after row t-1
+    (a [T, ld] tensor, or a column slice ``big[:, c0:c0+n]`` of one).  Enqueues on ``stream``."""
+    import torch
+    if x.dtype != torch.float32 or not x.is_cuda or not x.is_contiguous():
+        raise ValueError("x must be a contiguous CUDA float32 tensor")
+    if snr.dtype != torch.complex64 or not snr.is_cuda:
+        raise ValueError("snr must be a CUDA complex64 tensor")
+    n = int(x.numel()) if n is None else int(n)
+    if ld is None:
+        if snr.dim() != 2 or (snr.shape[1] > 1 and snr.stride(1) != 1) or snr.shape[1] < n:
+            raise ValueError("snr must be [T, >=n] with unit column stride")
+        ld = int(snr.stride(0)) if snr.shape[0] > 1 else max(int(snr.shape[1]), n)
+    _check(load_library().spiir_filter(bank, ctypes.c_void_p(x.data_ptr()), n, ctypes.c_void_p(snr.data_ptr()),
+                                       int(ld), _stream_handle(stream)))
+
+
+def spiir_filter_host(bank, x: np.ndarray, snr: np.ndarray | None = None) -> np.ndarray:
+    """Host-buffer entry: x float32 [n] numpy -> complex64 [T, n] numpy (H2D, kernels, D2H inside)."""
+    lib = load_library()
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    T = int(lib.spiir_bank_num_templates(bank))
+    if snr is None:
+        snr = np.empty((T, x.size), dtype=np.complex64)
+    if snr.dtype != np.complex64 or snr.ndim != 2 or snr.shape[0] != T or snr.shape[1] < x.size or \
+            (snr.shape[1] > 1 and snr.strides[1] != 8):
+        raise ValueError("snr must be complex64 [T, >=n] with unit column stride")
+    ld = snr.strides[0] // 8 if T > 1 else max(snr.shape[1], x.size)
+    _check(lib.spiir_filter_host(bank, _ptr(x), x.size, _ptr(snr), ld))
+    return snr
+
+
+def spiir_bank_reset(bank, stream=None):
+    _check(load_library().spiir_bank_reset(bank, _stream_handle(stream)))
+
+
+def spiir_bank_num_templates(bank) -> int:
+    return int(load_library().spiir_bank_num_templates(bank))
+
+
+def spiir_bank_num_filters(bank) -> int:
+    return int(load_library().spiir_bank_num_filters(bank))
+
+
+def spiir_bank_max_delay(bank) -> int:
+    return int(load_library().spiir_bank_max_delay(bank))
+
+
+def spiir_bank_last_path(bank) -> int:
+    return int(load_library().spiir_bank_last_path(bank))
+
+
+def spiir_bank_get_state(bank, y=None, hist=None, stream=None):
+    """y: CUDA complex64 [K] (caller's filter order); hist: CUDA float32 [D]; either may be None."""
+    _check(load_library().spiir_bank_get_state(bank, ctypes.c_void_p(y.data_ptr()) if y is not None else None,
+                                               ctypes.c_void_p(hist.data_ptr()) if hist is not None else None,
+                                               _stream_handle(stream)))
+
+
+def spiir_bank_set_state(bank, y=None, hist=None, stream=None):
+    _check(load_library().spiir_bank_set_state(bank, ctypes.c_void_p(y.data_ptr()) if y is not None else None,
+                                               ctypes.c_void_p(hist.data_ptr()) if hist is not None else None,
+                                               _stream_handle(stream)))
+
+
+def spiir_bank_destroy(bank):
+    _check(load_library().spiir_bank_destroy(bank))
+
+
+def spiir_kernel_launches() -> int:
+    return int(load_library().spiir_kernel_launches())
+
+
+def spiir_last_error() -> str:
+    return load_library().spiir_last_error().decode()
+
+
+def spiir_version() -> int:
+    return int(load_library().spiir_version())
+
+
+class SpiirBank:
+    """Convenience owner of a bank handle (context manager); still argument marshalling only."""
+
+    def __init__(self, filter_offsets, a1, b0, delays, device: int = 0, options: SpiirOptions | None = None):
+        self.handle = spiir_bank_create(filter_offsets, a1, b0, delays, device, options)
+        self.device = device
+        self.n_templates = spiir_bank_num_templates(self.handle)
+        self.n_filters = spiir_bank_num_filters(self.handle)
+        self.max_delay = spiir_bank_max_delay(self.handle)
+
+    def filter(self, x, snr=None, stream=None):
+        import torch
+        if snr is None:
+            snr = torch.empty((self.n_templates, x.numel()), dtype=torch.complex64, device=x.device)
+        spiir_filter(self.handle, x, snr, stream=stream)
+        return snr
+
+    def filter_host(self, x, snr=None):
+        return spiir_filter_host(self.handle, x, snr)
+
+    def reset(self, stream=None):
+        spiir_bank_reset(self.handle, stream)
+
+    @property
+    def last_path(self) -> int:
+        return spiir_bank_last_path(self.handle)
+
+    def close(self):
+        if self.handle is not None:
+            spiir_bank_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,525 @@
+// C ABI of the B200-native SPIIR template-bank filter: see include/spiir.h for the contract.
+// Host logic only (validation, bank layout upload, input tape, path choice, launches); every step of the
+// hot path runs in the kernels of spiir_kernels.cuh.  No CPU fallback exists.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/spiir.h"
+#include "spiir_kernels.cuh"
+
+using namespace spiir;
+
+namespace {
+
+thread_local char g_err[512] = "";
+std::atomic<int64_t> g_launches{0};
+
+int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU_TRY(expr)                                                                              \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(e_ == cudaErrorMemoryAllocation ? SPIIR_ENOMEM : SPIIR_ECUDA, "%s: %s", #expr, \
+                        cudaGetErrorString(e_));                                                  \
+    } while (0)
+
+constexpr size_t kPartBytes = 2ull * kWarpsPerCta * kTS * sizeof(u64);
+
+template <typename T>
+cudaError_t upload(T** dst, const std::vector<T>& v)
+{
+    *dst = nullptr;
+    const size_t bytes = std::max<size_t>(v.size(), 1) * sizeof(T);
+    cudaError_t e = cudaMalloc((void**)dst, bytes);
+    if (e != cudaSuccess) return e;
+    if (!v.empty()) e = cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+    return e;
+}
+
+}  // namespace
+
+struct spiir_bank {
+    int device = 0;
+    int F = 8;
+    int64_t T = 0, K = 0, D = 0, n_slots = 0, n_tiles = 0;
+    int32_t n_items = 0;
+    double avg_conflict_degree = 0.0;
+    spiir_options opt{};
+    // device bank
+    float *ar = nullptr, *ai2 = nullptr, *b = nullptr, *y = nullptr;
+    int32_t* dly = nullptr;
+    int32_t* item_round0 = nullptr;
+    WarpWork* work = nullptr;
+    int64_t* slot_of_filter = nullptr;
+    // input tape: tape[cur][0..pos) holds the most recent samples, the next chunk is appended at pos
+    float* tape[2] = {nullptr, nullptr};
+    int cur = 0;
+    int64_t cap = 0, pos = 0;
+    // scan scratch
+    float *zbuf = nullptr, *cbuf = nullptr;
+    int64_t scan_cap_seg = 0;
+    // host-path scratch
+    float *hx = nullptr, *hsnr = nullptr;
+    int64_t hx_cap = 0, hsnr_cap = 0;
+    cudaStream_t hstream = nullptr;
+    // device facts
+    int n_sm = 0;
+    size_t smem_optin = 0;
+    int32_t last_path = SPIIR_PATH_AUTO;
+    bool poisoned = false;
+    // occupancy cache (CTAs per SM for a given dynamic shared memory size)
+    size_t occ_smem[8] = {0};
+    int occ_val[8] = {0};
+    bool occ_gmem[8] = {false};
+    int occ_n = 0;
+};
+
+namespace {
+
+int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
+
+void free_bank(spiir_bank* bk)
+{
+    if (!bk) return;
+    cudaFree(bk->ar); cudaFree(bk->ai2); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
+    cudaFree(bk->item_round0); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
+    cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
+    cudaFree(bk->hx); cudaFree(bk->hsnr);
+    if (bk->hstream) cudaStreamDestroy(bk->hstream);
+    delete bk;
+}
+
+// (re)allocate the tape so that a chunk of n samples fits behind the history; keeps the history
+int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
+{
+    const int64_t need = round_up(bk->D, 4) + n + 16;
+    if (bk->cap >= need && bk->pos + n + 8 <= bk->cap) return SPIIR_OK;
+    const int64_t hist0 = round_up(bk->D, 4);
+    if (bk->cap < need) {
+        const int64_t cap = round_up(bk->D, 4) + std::max<int64_t>(4 * n, 1 << 16) + 16;
+        float* nt[2] = {nullptr, nullptr};
+        for (int i = 0; i < 2; ++i) CU_TRY(cudaMalloc((void**)&nt[i], (size_t)cap * sizeof(float)));
+        CU_TRY(cudaMemsetAsync(nt[0], 0, (size_t)cap * sizeof(float), st));
+        CU_TRY(cudaMemsetAsync(nt[1], 0, (size_t)cap * sizeof(float), st));
+        if (bk->tape[bk->cur] && bk->D > 0)
+            CU_TRY(cudaMemcpyAsync(nt[0] + hist0 - bk->D, bk->tape[bk->cur] + bk->pos - bk->D,
+                                   (size_t)bk->D * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        CU_TRY(cudaStreamSynchronize(st));
+        cudaFree(bk->tape[0]);
+        cudaFree(bk->tape[1]);
+        bk->tape[0] = nt[0];
+        bk->tape[1] = nt[1];
+        bk->cur = 0;
+        bk->cap = cap;
+        bk->pos = hist0;
+        return SPIIR_OK;
+    }
+    // compact: move the last D samples to the front of the other buffer
+    const int other = bk->cur ^ 1;
+    if (bk->D > 0)
+        CU_TRY(cudaMemcpyAsync(bk->tape[other] + hist0 - bk->D, bk->tape[bk->cur] + bk->pos - bk->D,
+                               (size_t)bk->D * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    bk->cur = other;
+    bk->pos = hist0;
+    return SPIIR_OK;
+}
+
+// allow the kernel to use all opt-in shared memory (once per instantiation and device)
+template <int F, bool G>
+int configure_kernel(int device, size_t smem_optin)
+{
+    static std::atomic<uint64_t> done_mask{0};
+    const uint64_t bit = 1ull << (device & 63);
+    if (done_mask.load(std::memory_order_acquire) & bit) return SPIIR_OK;
+    CU_TRY(cudaFuncSetAttribute(spiir_filter_kernel<F, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_optin));
+    done_mask.fetch_or(bit, std::memory_order_release);
+    return SPIIR_OK;
+}
+
+template <int F, bool G>
+int launch_one(const spiir_bank* bk, const FilterParams& p, dim3 grid, size_t smem, cudaStream_t st)
+{
+    int rc = configure_kernel<F, G>(bk->device, bk->smem_optin);
+    if (rc) return rc;
+    spiir_filter_kernel<F, G><<<grid, kThreads, smem, st>>>(p);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CU_TRY(cudaGetLastError());
+    return SPIIR_OK;
+}
+
+template <bool G>
+int launch_F(const spiir_bank* bk, const FilterParams& p, dim3 grid, size_t smem, cudaStream_t st)
+{
+    switch (bk->F) {
+        case 2: return launch_one<2, G>(bk, p, grid, smem, st);
+        case 4: return launch_one<4, G>(bk, p, grid, smem, st);
+        case 8: return launch_one<8, G>(bk, p, grid, smem, st);
+        case 16: return launch_one<16, G>(bk, p, grid, smem, st);
+    }
+    return fail(SPIIR_EINVAL, "unsupported filters_per_thread %d", bk->F);
+}
+
+template <int F, bool G>
+int occupancy_one(const spiir_bank* bk, size_t smem, int* occ)
+{
+    int rc = configure_kernel<F, G>(bk->device, bk->smem_optin);
+    if (rc) return rc;
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, spiir_filter_kernel<F, G>, kThreads, smem));
+    return SPIIR_OK;
+}
+
+int occupancy(const spiir_bank* bk, bool g, size_t smem, int* occ)
+{
+    switch (bk->F) {
+        case 2: return g ? occupancy_one<2, true>(bk, smem, occ) : occupancy_one<2, false>(bk, smem, occ);
+        case 4: return g ? occupancy_one<4, true>(bk, smem, occ) : occupancy_one<4, false>(bk, smem, occ);
+        case 8: return g ? occupancy_one<8, true>(bk, smem, occ) : occupancy_one<8, false>(bk, smem, occ);
+        case 16: return g ? occupancy_one<16, true>(bk, smem, occ) : occupancy_one<16, false>(bk, smem, occ);
+    }
+    return fail(SPIIR_EINVAL, "unsupported filters_per_thread %d", bk->F);
+}
+
+int cached_occupancy(spiir_bank* bk, bool g, size_t smem, int* occ)
+{
+    for (int i = 0; i < bk->occ_n; ++i)
+        if (bk->occ_smem[i] == smem && bk->occ_gmem[i] == g) { *occ = bk->occ_val[i]; return SPIIR_OK; }
+    int rc = occupancy(bk, g, smem, occ);
+    if (rc) return rc;
+    const int i = bk->occ_n < 8 ? bk->occ_n++ : 7;
+    bk->occ_smem[i] = smem; bk->occ_gmem[i] = g; bk->occ_val[i] = *occ;
+    return SPIIR_OK;
+}
+
+FilterParams base_params(const spiir_bank* bk)
+{
+    FilterParams p{};
+    p.ar = bk->ar; p.ai2 = bk->ai2; p.b = bk->b; p.dly = bk->dly;
+    p.item_round0 = bk->item_round0; p.work = bk->work; p.n_items = bk->n_items;
+    return p;
+}
+
+// Run the filter kernels over n samples whose window starts at xwin (aligned), sample 0 at xwin[w0].
+int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st)
+{
+    const size_t smem_cap = bk->smem_optin;
+    const int64_t max_win = ((int64_t)smem_cap - (int64_t)kPartBytes) / 4 - 8;   // floats
+    const bool gmem = (w0 + kTS > max_win);   // history alone does not fit: read x through L1/L2
+    int path = bk->opt.path;
+    // ---- how much time-parallelism is needed to fill the machine?
+    int64_t n_seg = 1;
+    if (path == SPIIR_PATH_SCAN || (path == SPIIR_PATH_AUTO && bk->n_items < bk->n_sm && n >= 4 * kTS)) {
+        const int64_t max_seg = std::max<int64_t>(1, n / kTS);
+        int64_t want = bk->opt.scan_segments > 0 ? bk->opt.scan_segments
+                                                 : ((int64_t)2 * bk->n_sm + bk->n_items - 1) / bk->n_items;
+        n_seg = std::min(std::max<int64_t>(want, 1), max_seg);
+        if (n_seg < 2 && path != SPIIR_PATH_SCAN) n_seg = 1;
+    }
+    if (n_seg <= 1) {
+        // ------------------------------------------------ sequential-in-time path
+        bk->last_path = (path == SPIIR_PATH_STREAM) ? SPIIR_PATH_STREAM : SPIIR_PATH_THROUGHPUT;
+        const int64_t sub = gmem ? n : std::max<int64_t>(kTS, (max_win - w0) / kTS * kTS);
+        for (int64_t off = 0; off < n; off += sub) {
+            const int64_t ns = std::min(sub, n - off);
+            FilterParams p = base_params(bk);
+            p.y_in = bk->y; p.y_out = bk->y; p.y_in_stride = 0; p.y_out_stride = 0; p.store_last_only = 1;
+            p.xwin = xwin + off; p.w0 = w0; p.n = ns; p.seg_len = ns;
+            p.snr = snr + 2 * off; p.ld = ld;
+            const size_t smem = gmem ? kPartBytes : (size_t)round_up(w0 + ns, 4) * 4 + kPartBytes;
+            int occ = 1;
+            int rc = cached_occupancy(bk, gmem, smem, &occ);
+            if (rc) return rc;
+            if (occ < 1) return fail(SPIIR_ECUDA, "filter kernel does not fit on an SM (smem %zu)", smem);
+            dim3 grid((unsigned)std::min<int64_t>(bk->n_items, (int64_t)bk->n_sm * occ), 1, 1);
+            rc = gmem ? launch_F<true>(bk, p, grid, smem, st) : launch_F<false>(bk, p, grid, smem, st);
+            if (rc) return rc;
+        }
+        return SPIIR_OK;
+    }
+    // ---------------------------------------------------- time-parallel scan path (north_star (4))
+    bk->last_path = SPIIR_PATH_SCAN;
+    int64_t seg_len = round_up((n + n_seg - 1) / n_seg, kTS);
+    if (!gmem && w0 + seg_len > max_win) seg_len = std::max<int64_t>(kTS, (max_win - w0) / kTS * kTS);
+    n_seg = (n + seg_len - 1) / seg_len;
+    if (n_seg > bk->scan_cap_seg) {
+        cudaFree(bk->zbuf); cudaFree(bk->cbuf);
+        bk->zbuf = bk->cbuf = nullptr;
+        bk->scan_cap_seg = 0;
+        const size_t bytes = (size_t)n_seg * 2 * bk->n_slots * sizeof(float);
+        CU_TRY(cudaMalloc((void**)&bk->zbuf, bytes));
+        CU_TRY(cudaMalloc((void**)&bk->cbuf, bytes));
+        bk->scan_cap_seg = n_seg;
+    }
+    const size_t smem = gmem ? kPartBytes : (size_t)round_up(w0 + seg_len, 4) * 4 + kPartBytes;
+    int occ = 1;
+    int rc = cached_occupancy(bk, gmem, smem, &occ);
+    if (rc) return rc;
+    if (occ < 1) return fail(SPIIR_ECUDA, "filter kernel does not fit on an SM (smem %zu)", smem);
+    const unsigned gx = (unsigned)bk->n_items;
+    if (n_seg > 1) {
+        // pass 1: zero-state end values of segments 0 .. n_seg-2 (no sums, no output)
+        FilterParams p = base_params(bk);
+        p.y_in = nullptr; p.y_out = bk->zbuf; p.y_out_stride = 2 * bk->n_slots; p.store_last_only = 0;
+        p.xwin = xwin; p.w0 = w0; p.n = (n_seg - 1) * seg_len; p.seg_len = seg_len;
+        p.snr = nullptr; p.ld = 0;
+        dim3 grid(gx, (unsigned)(n_seg - 1), 1);
+        rc = gmem ? launch_F<true>(bk, p, grid, smem, st) : launch_F<false>(bk, p, grid, smem, st);
+        if (rc) return rc;
+    }
+    {
+        // carry scan: c_0 = y, c_{q+1} = a1^seg_len c_q + z_q   (double precision)
+        const int threads = 256;
+        const unsigned blocks = (unsigned)((bk->n_slots + threads - 1) / threads);
+        spiir_scan_carry_kernel<<<blocks, threads, 0, st>>>(bk->ar, bk->ai2, bk->y, bk->zbuf, bk->cbuf,
+                                                            bk->n_slots, (int32_t)n_seg, seg_len);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        CU_TRY(cudaGetLastError());
+    }
+    {
+        // pass 2: every segment from its true start state, full sums and output; last segment stores y
+        FilterParams p = base_params(bk);
+        p.y_in = bk->cbuf; p.y_in_stride = 2 * bk->n_slots; p.y_out = bk->y; p.y_out_stride = 0; p.store_last_only = 1;
+        p.xwin = xwin; p.w0 = w0; p.n = n; p.seg_len = seg_len;
+        p.snr = snr; p.ld = ld;
+        dim3 grid(gx, (unsigned)n_seg, 1);
+        rc = gmem ? launch_F<true>(bk, p, grid, smem, st) : launch_F<false>(bk, p, grid, smem, st);
+        if (rc) return rc;
+    }
+    return SPIIR_OK;
+}
+
+int choose_F(int32_t T, const int64_t* off, int requested)
+{
+    if (requested == 2 || requested == 4 || requested == 8 || requested == 16) return requested;
+    // least padded work; F = 8 is the fastest inner loop, F = 4 pays ~4 % more reduction overhead
+    double best = 0;
+    int bestF = 8;
+    for (int F : {8, 4}) {
+        const int64_t per = 32LL * F;
+        double padded = 0;
+        for (int32_t t = 0; t < T; ++t) padded += (double)((off[t + 1] - off[t] + per - 1) / per * per);
+        padded *= (F == 8 ? 1.0 : 1.04);
+        if (bestF == 8 && F == 8) { best = padded; continue; }
+        if (padded < best) { best = padded; bestF = F; }
+    }
+    return bestF;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* spiir_last_error(void) { return g_err; }
+int64_t spiir_kernel_launches(void) { return g_launches.load(); }
+int32_t spiir_version(void) { return 100; }
+
+int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const float* a1, const float* b0,
+                      const int32_t* delays, int32_t device, const spiir_options* opt)
+{
+    if (out) *out = nullptr;
+    if (!out || !off || !a1 || !b0 || !delays) return fail(SPIIR_EINVAL, "null argument");
+    if (T <= 0) return fail(SPIIR_EINVAL, "n_templates must be >= 1");
+    if (off[0] != 0) return fail(SPIIR_EINVAL, "filter_offsets[0] must be 0");
+    for (int32_t t = 0; t < T; ++t)
+        if (off[t + 1] <= off[t]) return fail(SPIIR_EINVAL, "template %d has no filters (offsets must increase)", t);
+    const int64_t K = off[T];
+    int64_t D = 0;
+    for (int64_t k = 0; k < K; ++k) {
+        const float re = a1[2 * k], im = a1[2 * k + 1];
+        if (!std::isfinite(re) || !std::isfinite(im) || !std::isfinite(b0[2 * k]) || !std::isfinite(b0[2 * k + 1]))
+            return fail(SPIIR_EINVAL, "non-finite coefficient at filter %lld", (long long)k);
+        if ((double)re * re + (double)im * im >= 1.0) return fail(SPIIR_EINVAL, "|a1| >= 1 at filter %lld", (long long)k);
+        if (delays[k] < 0) return fail(SPIIR_EINVAL, "negative delay at filter %lld", (long long)k);
+        D = std::max<int64_t>(D, delays[k]);
+    }
+    spiir_options o{};
+    o.struct_size = (int32_t)sizeof(o);
+    if (opt) {
+        if (opt->struct_size < (int32_t)(4 * sizeof(int32_t))) return fail(SPIIR_EINVAL, "bad spiir_options.struct_size");
+        memcpy(&o, opt, std::min<size_t>((size_t)opt->struct_size, sizeof(o)));
+        if (o.path < SPIIR_PATH_AUTO || o.path > SPIIR_PATH_STREAM) return fail(SPIIR_EINVAL, "bad path option");
+        if (o.filters_per_thread != 0 && o.filters_per_thread != 2 && o.filters_per_thread != 4 &&
+            o.filters_per_thread != 8 && o.filters_per_thread != 16)
+            return fail(SPIIR_EINVAL, "filters_per_thread must be 0, 2, 4, 8 or 16");
+        if (o.scan_segments < 0) return fail(SPIIR_EINVAL, "scan_segments must be >= 0");
+    }
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0)
+        return fail(SPIIR_ECUDA, "no CUDA device available (this library has no CPU fallback)");
+    if (device < 0 || device >= n_dev) return fail(SPIIR_EINVAL, "device %d out of range", device);
+    CU_TRY(cudaSetDevice(device));
+
+    spiir_bank* bk = new (std::nothrow) spiir_bank();
+    if (!bk) return fail(SPIIR_ENOMEM, "out of host memory");
+    bk->device = device;
+    bk->opt = o;
+    bk->T = T; bk->K = K; bk->D = D;
+    bk->F = choose_F(T, off, o.filters_per_thread);
+    HostLayout L;
+    try {
+        L = build_layout(T, off, a1, b0, delays, bk->F);
+    } catch (const std::bad_alloc&) {
+        free_bank(bk);
+        return fail(SPIIR_ENOMEM, "out of host memory building the bank layout");
+    }
+    bk->n_slots = L.n_slots;
+    bk->n_tiles = L.n_tiles;
+    bk->n_items = (int32_t)(L.item_round0.size() - 1);
+    bk->avg_conflict_degree = L.avg_conflict_degree;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDeviceProperties(&prop, device);
+    if (e == cudaSuccess) {
+        bk->n_sm = prop.multiProcessorCount;
+        bk->smem_optin = prop.sharedMemPerBlockOptin;
+    }
+    if (e == cudaSuccess) e = upload(&bk->ar, L.ar);
+    if (e == cudaSuccess) e = upload(&bk->ai2, L.ai2);
+    if (e == cudaSuccess) e = upload(&bk->b, L.b);
+    if (e == cudaSuccess) e = upload(&bk->dly, L.dly);
+    if (e == cudaSuccess) e = upload(&bk->item_round0, L.item_round0);
+    if (e == cudaSuccess) e = upload(&bk->work, L.work);
+    if (e == cudaSuccess) e = upload(&bk->slot_of_filter, L.slot_of_filter);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&bk->y, (size_t)std::max<int64_t>(L.n_slots, 1) * 2 * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemset(bk->y, 0, (size_t)std::max<int64_t>(L.n_slots, 1) * 2 * sizeof(float));
+    if (e != cudaSuccess) {
+        free_bank(bk);
+        return fail(e == cudaErrorMemoryAllocation ? SPIIR_ENOMEM : SPIIR_ECUDA, "bank upload: %s", cudaGetErrorString(e));
+    }
+    int rc = ensure_tape(bk, 1 << 14, nullptr);
+    if (rc == SPIIR_OK) {
+        e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) rc = fail(SPIIR_ECUDA, "bank create: %s", cudaGetErrorString(e));
+    }
+    if (rc != SPIIR_OK) { free_bank(bk); return rc; }
+    *out = bk;
+    return SPIIR_OK;
+}
+
+int spiir_filter(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, int64_t ld, void* stream)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    if (bk->poisoned) return fail(SPIIR_ESTATE, "bank unusable after an earlier failure");
+    if (n < 0 || ld < n) return fail(SPIIR_EINVAL, "need 0 <= n <= ld");
+    if (n == 0) return SPIIR_OK;
+    if (!x_dev || !snr_dev) return fail(SPIIR_EINVAL, "null device pointer");
+    if (n > (int64_t)1 << 30) return fail(SPIIR_EINVAL, "chunk too long");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(cudaSetDevice(bk->device));
+    int rc = ensure_tape(bk, n, st);
+    if (rc) return rc;
+    float* tape = bk->tape[bk->cur];
+    CU_TRY(cudaMemcpyAsync(tape + bk->pos, x_dev, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    const int64_t start_al = (bk->pos - bk->D) / 4 * 4;
+    const int w0 = (int)(bk->pos - start_al);
+    rc = run_chunk(bk, tape + start_al, w0, n, snr_dev, ld, st);
+    if (rc) { bk->poisoned = true; return rc; }
+    bk->pos += n;
+    return SPIIR_OK;
+}
+
+int spiir_filter_host(spiir_bank* bk, const float* x_host, int64_t n, float* snr_host, int64_t ld)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    if (n < 0 || ld < n) return fail(SPIIR_EINVAL, "need 0 <= n <= ld");
+    if (n == 0) return SPIIR_OK;
+    if (!x_host || !snr_host) return fail(SPIIR_EINVAL, "null host pointer");
+    CU_TRY(cudaSetDevice(bk->device));
+    if (!bk->hstream) CU_TRY(cudaStreamCreateWithFlags(&bk->hstream, cudaStreamNonBlocking));
+    if (bk->hx_cap < n) {
+        cudaFree(bk->hx); bk->hx = nullptr; bk->hx_cap = 0;
+        CU_TRY(cudaMalloc((void**)&bk->hx, (size_t)n * sizeof(float)));
+        bk->hx_cap = n;
+    }
+    const int64_t need = bk->T * n * 2;
+    if (bk->hsnr_cap < need) {
+        cudaFree(bk->hsnr); bk->hsnr = nullptr; bk->hsnr_cap = 0;
+        CU_TRY(cudaMalloc((void**)&bk->hsnr, (size_t)need * sizeof(float)));
+        bk->hsnr_cap = need;
+    }
+    CU_TRY(cudaMemcpyAsync(bk->hx, x_host, (size_t)n * sizeof(float), cudaMemcpyHostToDevice, bk->hstream));
+    int rc = spiir_filter(bk, bk->hx, n, bk->hsnr, n, bk->hstream);
+    if (rc) return rc;
+    CU_TRY(cudaMemcpy2DAsync(snr_host, (size_t)ld * 8, bk->hsnr, (size_t)n * 8, (size_t)n * 8, (size_t)bk->T,
+                             cudaMemcpyDeviceToHost, bk->hstream));
+    CU_TRY(cudaStreamSynchronize(bk->hstream));
+    return SPIIR_OK;
+}
+
+int spiir_bank_reset(spiir_bank* bk, void* stream)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(cudaSetDevice(bk->device));
+    CU_TRY(cudaMemsetAsync(bk->y, 0, (size_t)std::max<int64_t>(bk->n_slots, 1) * 2 * sizeof(float), st));
+    bk->pos = round_up(bk->D, 4);
+    CU_TRY(cudaMemsetAsync(bk->tape[bk->cur], 0, (size_t)(bk->pos + 8) * sizeof(float), st));
+    bk->poisoned = false;
+    return SPIIR_OK;
+}
+
+int64_t spiir_bank_num_templates(const spiir_bank* bk) { return bk ? bk->T : -1; }
+int64_t spiir_bank_num_filters(const spiir_bank* bk) { return bk ? bk->K : -1; }
+int64_t spiir_bank_max_delay(const spiir_bank* bk) { return bk ? bk->D : -1; }
+int32_t spiir_bank_last_path(const spiir_bank* bk) { return bk ? bk->last_path : -1; }
+
+int spiir_bank_get_state(spiir_bank* bk, float* y_dev, float* hist_dev, void* stream)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(cudaSetDevice(bk->device));
+    if (y_dev) {
+        const int threads = 256;
+        spiir_permute_state_kernel<<<(unsigned)((bk->K + threads - 1) / threads), threads, 0, st>>>(
+            bk->y, y_dev, bk->slot_of_filter, bk->K, 0);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        CU_TRY(cudaGetLastError());
+    }
+    if (hist_dev && bk->D > 0)
+        CU_TRY(cudaMemcpyAsync(hist_dev, bk->tape[bk->cur] + bk->pos - bk->D, (size_t)bk->D * sizeof(float),
+                               cudaMemcpyDeviceToDevice, st));
+    return SPIIR_OK;
+}
+
+int spiir_bank_set_state(spiir_bank* bk, const float* y_dev, const float* hist_dev, void* stream)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(cudaSetDevice(bk->device));
+    if (y_dev) {
+        const int threads = 256;
+        spiir_permute_state_kernel<<<(unsigned)((bk->K + threads - 1) / threads), threads, 0, st>>>(
+            y_dev, bk->y, bk->slot_of_filter, bk->K, 1);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        CU_TRY(cudaGetLastError());
+    }
+    if (hist_dev && bk->D > 0)
+        CU_TRY(cudaMemcpyAsync(bk->tape[bk->cur] + bk->pos - bk->D, hist_dev, (size_t)bk->D * sizeof(float),
+                               cudaMemcpyDeviceToDevice, st));
+    return SPIIR_OK;
+}
+
+int spiir_bank_destroy(spiir_bank* bk)
+{
+    if (!bk) return SPIIR_OK;
+    cudaSetDevice(bk->device);
+    cudaDeviceSynchronize();
+    free_bank(bk);
+    return SPIIR_OK;
+}
+
+}  // extern "C"

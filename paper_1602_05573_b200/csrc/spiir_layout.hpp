@@ -1,0 +1,200 @@
+// Host-side bank layout for the SPIIR filter kernels (north_star subsystem (1)
+// "parameter array ... aligned and continuous ... coalesed memory access").
+//
+// A template's filters are sorted by delay, then dealt to "groups" of 32 (one filter per lane of a
+// warp for one register slot f).  All 32 lanes of a group read x[n - d] from shared memory in the same
+// instruction, so the group is conflict-free iff its delays are distinct modulo 32 (or equal).  The
+// dealing first builds as many perfect groups as the residue histogram allows and spreads the rest
+// evenly, which keeps the average conflict degree near 1.4 for uniformly random delays (3.4 undealt).
+// F consecutive groups form a warp tile (32 lanes x F register slots); tiles are padded with null
+// filters (a1 = b0 = 0) whose delay copies a real filter of the same group (same address = broadcast).
+//
+// The layout of a template is a pure function of that template's own (a1, b0, d) arrays, so results are
+// bitwise independent of the template's position in the bank (invariants).
+#pragma once
+#include <algorithm>
+#include <cstdint>
+#include <numeric>
+#include <vector>
+
+namespace spiir {
+
+constexpr int kWarp = 32;
+constexpr int kWarpsPerCta = 8;   // W: warps of one CTA = warp tiles processed side by side
+
+struct WarpWork {        // what one warp does in one round of one CTA item
+    int32_t tile;        // warp tile index into the slot arrays, -1 = idle
+    int32_t row;         // template index = SNR row
+    int32_t first;       // first warp of this template in the round
+    int32_t count;       // number of warps of this template in the round
+};
+
+struct HostLayout {
+    int F = 0;                          // register slots (filters) per thread
+    int64_t n_tiles = 0;                // warp tiles
+    int64_t n_slots = 0;                // n_tiles * F * 32
+    std::vector<float> ar;              // [n_slots] Re a1
+    std::vector<float> ai2;             // [2*n_slots] (-Im a1, +Im a1) pairs for the packed complex FMA
+    std::vector<float> b;               // [2*n_slots] (Re b0, Im b0)
+    std::vector<int32_t> dly;           // [n_slots]
+    std::vector<int64_t> slot_of_filter;  // [K] caller's filter index -> slot
+    std::vector<int64_t> tile_begin;    // [T+1] first tile of each template
+    // work list: items (one CTA at a time), each with >= 1 rounds of kWarpsPerCta warp entries
+    std::vector<int32_t> item_round0;   // [n_items+1] first round of each item
+    std::vector<WarpWork> work;         // [n_rounds * kWarpsPerCta]
+    double avg_conflict_degree = 0.0;   // mean over groups of max residue multiplicity (diagnostic)
+};
+
+// Deal the delay-sorted filters `order` (indices into d) of one template into G groups of <= 32.
+// Returns group-major list: out[g] = filter indices of group g.
+inline void deal_groups(const int32_t* d, const std::vector<int64_t>& order, int G,
+                        std::vector<std::vector<int64_t>>& out, double& degree_sum)
+{
+    out.assign(G, {});
+    std::vector<std::vector<int64_t>> bucket(kWarp);
+    for (int64_t k : order) bucket[d[k] & 31].push_back(k);
+    std::vector<size_t> head(kWarp, 0);
+    const int64_t K = (int64_t)order.size();
+    // phase 1: perfect groups (one filter of every residue), only full groups of 32
+    size_t perfect = bucket[0].size();
+    for (int r = 1; r < kWarp; ++r) perfect = std::min(perfect, bucket[r].size());
+    perfect = std::min<size_t>(perfect, (size_t)(K / kWarp));
+    perfect = std::min<size_t>(perfect, (size_t)G);
+    for (size_t g = 0; g < perfect; ++g)
+        for (int r = 0; r < kWarp; ++r) out[g].push_back(bucket[r][head[r]++]);
+    // phase 2: spread the remainder evenly over the remaining groups: least multiplicity of the
+    // residue first, then emptiest group, then lowest index; fullest residues first
+    const int G2 = G - (int)perfect;
+    if (G2 > 0) {
+        std::vector<int> rorder(kWarp);
+        std::iota(rorder.begin(), rorder.end(), 0);
+        std::stable_sort(rorder.begin(), rorder.end(), [&](int a, int b) {
+            return bucket[a].size() - head[a] > bucket[b].size() - head[b];
+        });
+        std::vector<int> fill(G2, 0);
+        std::vector<int> mult((size_t)G2 * kWarp, 0);
+        // capacity per group: groups before the last tile's padding must be full; give every group
+        // ceil/floor share so padding lands in the last groups
+        const int64_t rem = K - (int64_t)perfect * kWarp;
+        std::vector<int> cap(G2, 0);
+        {
+            int64_t left = rem;
+            for (int g = 0; g < G2; ++g) { cap[g] = (int)std::min<int64_t>(kWarp, left); left -= cap[g]; }
+        }
+        for (int r : rorder) {
+            while (head[r] < bucket[r].size()) {
+                int best = -1;
+                for (int g = 0; g < G2; ++g) {
+                    if (fill[g] >= cap[g]) continue;
+                    if (best < 0 || mult[(size_t)g * kWarp + r] < mult[(size_t)best * kWarp + r] ||
+                        (mult[(size_t)g * kWarp + r] == mult[(size_t)best * kWarp + r] && fill[g] < fill[best]))
+                        best = g;
+                }
+                out[perfect + best].push_back(bucket[r][head[r]++]);
+                ++fill[best];
+                ++mult[(size_t)best * kWarp + r];
+            }
+        }
+    }
+    for (int g = 0; g < G; ++g) {
+        int cnt[kWarp] = {0};
+        int mx = 0;
+        for (int64_t k : out[g]) mx = std::max(mx, ++cnt[d[k] & 31]);
+        degree_sum += out[g].empty() ? 0 : mx;
+    }
+}
+
+inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, const float* b0,
+                               const int32_t* d, int F)
+{
+    HostLayout L;
+    L.F = F;
+    const int64_t K = off[T];
+    L.tile_begin.resize((size_t)T + 1);
+    int64_t tiles = 0;
+    const int64_t per_tile = (int64_t)kWarp * F;
+    for (int32_t t = 0; t < T; ++t) {
+        L.tile_begin[t] = tiles;
+        tiles += (off[t + 1] - off[t] + per_tile - 1) / per_tile;
+    }
+    L.tile_begin[T] = tiles;
+    L.n_tiles = tiles;
+    L.n_slots = tiles * per_tile;
+    L.ar.assign((size_t)L.n_slots, 0.f);
+    L.ai2.assign((size_t)L.n_slots * 2, 0.f);
+    L.b.assign((size_t)L.n_slots * 2, 0.f);
+    L.dly.assign((size_t)L.n_slots, 0);
+    L.slot_of_filter.assign((size_t)K, -1);
+
+    double degree_sum = 0.0;
+    int64_t n_groups = 0;
+    std::vector<int64_t> order;
+    std::vector<std::vector<int64_t>> groups;
+    for (int32_t t = 0; t < T; ++t) {
+        const int64_t k0 = off[t], Kt = off[t + 1] - off[t];
+        order.resize((size_t)Kt);
+        std::iota(order.begin(), order.end(), k0);
+        std::stable_sort(order.begin(), order.end(), [&](int64_t x, int64_t y) { return d[x] < d[y]; });
+        const int64_t nt = L.tile_begin[t + 1] - L.tile_begin[t];
+        const int G = (int)(nt * F);
+        deal_groups(d, order, G, groups, degree_sum);
+        for (int g = 0; g < G; ++g) {
+            if (groups[g].empty()) continue;
+            ++n_groups;
+            // lanes in delay order inside the group (any order is equally conflict-free)
+            const int64_t slot0 = (L.tile_begin[t] * F + g) * kWarp;
+            for (size_t l = 0; l < groups[g].size(); ++l) {
+                const int64_t k = groups[g][l], s = slot0 + (int64_t)l;
+                L.ar[s] = a1[2 * k];
+                L.ai2[2 * s] = -a1[2 * k + 1];
+                L.ai2[2 * s + 1] = a1[2 * k + 1];
+                L.b[2 * s] = b0[2 * k];
+                L.b[2 * s + 1] = b0[2 * k + 1];
+                L.dly[s] = d[k];
+                L.slot_of_filter[k] = s;
+            }
+            for (size_t l = groups[g].size(); l < (size_t)kWarp; ++l)   // null filters: broadcast read
+                L.dly[slot0 + (int64_t)l] = d[groups[g][0]];
+        }
+        // entirely empty groups of the last tile: point them at the template's smallest delay
+        for (int g = 0; g < G; ++g)
+            if (groups[g].empty())
+                for (int l = 0; l < kWarp; ++l) L.dly[(L.tile_begin[t] * F + g) * kWarp + l] = d[order[0]];
+    }
+    L.avg_conflict_degree = n_groups ? degree_sum / (double)n_groups : 0.0;
+
+    // Work list.  Templates with <= W tiles share an item round with their neighbours (greedy, in bank
+    // order); a template with more tiles gets an item of its own with several accumulate rounds.
+    const int W = kWarpsPerCta;
+    L.item_round0.push_back(0);
+    std::vector<WarpWork> cur;
+    auto flush = [&]() {
+        if (cur.empty()) return;
+        while ((int)cur.size() < W) cur.push_back(WarpWork{-1, 0, 0, 0});
+        L.work.insert(L.work.end(), cur.begin(), cur.end());
+        L.item_round0.push_back((int32_t)(L.work.size() / W));
+        cur.clear();
+    };
+    for (int32_t t = 0; t < T; ++t) {
+        const int64_t nt = L.tile_begin[t + 1] - L.tile_begin[t];
+        if (nt <= W) {
+            if ((int64_t)cur.size() + nt > W) flush();
+            const int first = (int)cur.size();
+            for (int64_t i = 0; i < nt; ++i)
+                cur.push_back(WarpWork{(int32_t)(L.tile_begin[t] + i), t, first, (int32_t)nt});
+        } else {
+            flush();
+            for (int64_t i0 = 0; i0 < nt; i0 += W) {
+                const int cnt = (int)std::min<int64_t>(W, nt - i0);
+                for (int i = 0; i < W; ++i)
+                    L.work.push_back(i < cnt ? WarpWork{(int32_t)(L.tile_begin[t] + i0 + i), t, 0, cnt}
+                                             : WarpWork{-1, 0, 0, 0});
+            }
+            L.item_round0.push_back((int32_t)(L.work.size() / W));
+        }
+    }
+    flush();
+    return L;
+}
+
+}  // namespace spiir

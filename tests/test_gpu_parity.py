@@ -1,0 +1,261 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded float32 inputs.  Acceptance (BASELINE.json:north_star): per template
+    max_n |SNR_gpu - SNR_ref| <= 1e-4 * max_n |SNR_ref|
+for one-shot and for every chunked run; the dyadic golden vector P7 must match bitwise.
+"""
+from fractions import Fraction
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+import spiir_inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4   # north_star tolerance, relative to the template's max |SNR_ref|
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    import oracle
+    import paper_1602_05573_b200 as pkg
+    pkg.load_library()
+    return pkg, oracle, torch
+
+
+def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=False):
+    """Filter inp.x through a fresh bank in the given chunking; returns complex64 [T or len(rows), N]."""
+    pkg, _, torch = env
+    N = inp.n_samples
+    chunks = [N] if chunks is None else list(chunks)
+    assert sum(chunks) == N
+    opt = pkg.SpiirOptions(path=path, filters_per_thread=F, scan_segments=segments)
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank:
+        if host:
+            out = np.empty((inp.n_templates, N), dtype=np.complex64)
+            pos = 0
+            for c in chunks:
+                pkg.spiir_filter_host(bank.handle, inp.x[pos:pos + c], out[:, pos:pos + c])
+                pos += c
+            return out if rows is None else out[rows]
+        x = torch.from_numpy(inp.x).cuda()
+        snr = torch.full((inp.n_templates, N), float("nan"), dtype=torch.complex64, device="cuda")
+        pos = 0
+        for c in chunks:
+            if c > 0:
+                pkg.spiir_filter(bank.handle, x[pos:pos + c], snr[:, pos:pos + c])
+            else:
+                pkg.spiir_filter(bank.handle, x[pos:pos], snr[:, pos:pos], ld=N, n=0)
+            pos += c
+        torch.cuda.synchronize()
+        sel = snr if rows is None else snr[torch.as_tensor(np.asarray(rows), device="cuda")]
+        return sel.cpu().numpy()
+
+
+def rel_err(got, ref):
+    got = got.astype(np.complex128)
+    scale = np.abs(ref).max(axis=1)
+    scale = np.where(scale > 0, scale, 1.0)
+    return np.abs(got - ref).max(axis=1) / scale
+
+
+def check(got, ref, tol=TOL):
+    assert got.shape == ref.shape
+    assert np.isfinite(got.view(np.float32)).all(), "GPU output has non-finite or unwritten entries"
+    err = rel_err(got, ref)
+    assert err.max() <= tol, f"max relative error {err.max():.3e} at template {int(err.argmax())}"
+    return err.max()
+
+
+# ------------------------------------------------------------------ exact golden vector, all paths
+@pytest.mark.parametrize("path,F", [(1, 0), (1, 2), (1, 16), (2, 0)])
+def test_p7_golden_vector_bitwise(env, path, F):
+    rows, filters, x = [], [], None
+    for line in (Path(__file__).parent / "golden" / "p7_dyadic.txt").read_text().splitlines():
+        if line.startswith("# x:"):
+            x = np.array([int(v) for v in line[4:].split()], dtype=np.float32)
+        elif line.startswith("#"):
+            parts = line[1:].split()
+            if len(parts) == 5:
+                try:
+                    filters.append([Fraction(p) for p in parts])
+                except ValueError:
+                    pass
+        elif line.strip():
+            _, re, im = line.split()
+            rows.append(complex(float(Fraction(re)), float(Fraction(im))))
+    inp = spiir_inputs.SpiirInputs(
+        "p7", np.array([0, 3], np.int64),
+        np.array([complex(float(f[0]), float(f[1])) for f in filters], np.complex64),
+        np.array([complex(float(f[2]), float(f[3])) for f in filters], np.complex64),
+        np.array([int(f[4]) for f in filters], np.int32), x, 8)
+    got = run_gpu(env, inp, path=path, F=F)
+    assert np.array_equal(got[0], np.array(rows, dtype=np.complex64))
+    got = run_gpu(env, inp, chunks=[3, 1, 4], path=path, F=F)
+    assert np.array_equal(got[0], np.array(rows, dtype=np.complex64))
+
+
+# ------------------------------------------------------------------ configs 0 and 1, full bank, every element
+@pytest.mark.parametrize("path", [0, 1, 2])
+def test_cfg0_full(env, path):
+    inp = spiir_inputs.make_config(0)
+    ref = env[1].run_inputs(inp)
+    check(run_gpu(env, inp, path=path), ref)
+    check(run_gpu(env, inp, chunks=[1000, 24, 3000, 72], path=path), ref)
+
+
+@pytest.mark.parametrize("path", [0, 1, 2])
+def test_cfg1_full_oneshot_and_streaming(env, path):
+    inp = spiir_inputs.make_config(1)
+    ref = env[1].run_inputs(inp)
+    one = run_gpu(env, inp, path=path)
+    check(one, ref)
+    chunked = run_gpu(env, inp, chunks=[4096] * 16, path=path)
+    check(chunked, ref)
+    # streaming output equals one-shot output within the stated tolerance
+    assert rel_err(chunked, one.astype(np.complex128)).max() <= TOL
+
+
+def test_ragged_chunks_and_carry(env):
+    inp = spiir_inputs.make_config(1, n_templates=5, n_samples=3 * 4096 + 11)
+    D = inp.max_delay
+    ref = env[1].run_inputs(inp)
+    chunks = [1, 7, 0, 4096, D - 1, D + 1, 63, 65]
+    chunks.append(inp.n_samples - sum(chunks))
+    for path in (1, 2):
+        check(run_gpu(env, inp, chunks=chunks, path=path), ref)
+
+
+# ------------------------------------------------------------------ shapes: ragged templates, F variants, big templates
+@pytest.mark.parametrize("F", [2, 4, 8, 16])
+def test_ragged_templates_all_register_blockings(env, F):
+    counts = [1, 31, 32, 33, 64, 100, 255, 256, 257, 700, 5000, 3]
+    inp = spiir_inputs.make_random_bank(77, counts, 1500, d_max=300)
+    ref = env[1].run_inputs(inp)
+    check(run_gpu(env, inp, path=1, F=F), ref)
+    check(run_gpu(env, inp, chunks=[500, 9, 991], path=2, F=F, segments=5), ref)
+
+
+def test_zero_delay_and_constant_delay(env):
+    rng = np.random.default_rng(5)
+    inp = spiir_inputs.make_random_bank(6, [128, 40], 700, d_max=0)
+    assert inp.max_delay == 0
+    check(run_gpu(env, inp, path=1), env[1].run_inputs(inp))
+    inp2 = spiir_inputs.make_random_bank(7, [96], 700, d_max=50)
+    inp2.delays[:] = 32                           # every lane hits the same address (broadcast)
+    check(run_gpu(env, inp2, path=1), env[1].run_inputs(inp2))
+    inp3 = spiir_inputs.make_random_bank(8, [96], 700, d_max=50)
+    inp3.delays[:] = (rng.integers(0, 4, 96) * 32).astype(np.int32)   # worst-case bank conflicts
+    check(run_gpu(env, inp3, path=1), env[1].run_inputs(inp3))
+
+
+def test_history_longer_than_shared_memory(env):
+    # max delay 70 000 samples: the window cannot live in shared memory -> global-memory variant
+    inp = spiir_inputs.make_random_bank(9, [300, 64], 9000, d_max=70000)
+    inp.delays[0] = 70000
+    inp.delays[1] = 0
+    xlong = np.random.default_rng(10).standard_normal(80000).astype(np.float32)
+    inp = spiir_inputs.SpiirInputs(inp.name, inp.offsets, inp.a1, inp.b0, inp.delays, xlong, 80000)
+    ref = env[1].run_inputs(inp)
+    check(run_gpu(env, inp, chunks=[30000, 50000], path=1), ref)
+    check(run_gpu(env, inp, chunks=[30000, 50000], path=2), ref)
+
+
+def test_window_split_over_several_launches(env):
+    # D + n exceeds one shared-memory window: the call is split into sub-launches
+    inp = spiir_inputs.make_random_bank(11, [256, 256], 150000, d_max=20000)
+    ref = env[1].run_inputs(inp)
+    check(run_gpu(env, inp, path=1), ref)
+    check(run_gpu(env, inp, path=2), ref)
+
+
+# ------------------------------------------------------------------ config 2 (chirp structure), streaming, sampled templates
+def test_cfg2_streaming_subset(env):
+    inp = spiir_inputs.make_config(2)
+    rows = spiir_inputs.parity_subset(inp.n_templates, 24, 2)
+    ref = env[1].run_inputs(inp.select_templates(rows))
+    got = run_gpu(env, inp, chunks=[4096] * 16, rows=rows)
+    check(got, ref)
+
+
+# ------------------------------------------------------------------ config 3 (headline) at full size, launch config of bench.py
+def test_cfg3_full_size_subset_and_invariants(env):
+    pkg, oracle, torch = env
+    inp = spiir_inputs.make_config(3)
+    T = inp.n_templates
+    rows = spiir_inputs.parity_subset(T, 6, 3)
+    # plant copies of checked templates at other positions: must come out bitwise equal to their originals
+    src = rows[:3]
+    dst = np.array([17, 2048, T - 2])
+    K = 1024
+    for s, d in zip(src, dst):
+        inp.a1[d * K:(d + 1) * K] = inp.a1[s * K:(s + 1) * K]
+        inp.b0[d * K:(d + 1) * K] = inp.b0[s * K:(s + 1) * K]
+        inp.delays[d * K:(d + 1) * K] = inp.delays[s * K:(s + 1) * K]
+    all_rows = np.concatenate([rows, dst])
+    got = run_gpu(env, inp, chunks=[16384] * 16, rows=all_rows)
+    ref = oracle.run_inputs(inp.select_templates(rows))
+    check(got[:len(rows)], ref)
+    for i in range(3):
+        assert np.array_equal(got[i].view(np.float32), got[len(rows) + i].view(np.float32))
+
+
+# ------------------------------------------------------------------ config 4: variable filter counts, 16-sample chunks
+@pytest.mark.parametrize("path", [0, 2])
+def test_cfg4_tiny_chunks(env, path):
+    inp = spiir_inputs.make_config(4, n_templates=512, n_samples=1024)
+    kt = np.diff(inp.offsets)
+    order = np.argsort(kt)
+    rows = np.sort(order[np.linspace(0, len(order) - 1, 16).astype(int)])   # stratified over filter count
+    ref = env[1].run_inputs(inp.select_templates(rows))
+    got = run_gpu(env, inp, chunks=[16] * 64, path=path, rows=rows)
+    check(got, ref)
+
+
+# ------------------------------------------------------------------ oracle-free invariants
+def test_template_permutation_equivariance_and_determinism(env):
+    inp = spiir_inputs.make_random_bank(21, [256, 100, 512, 33, 256, 1024, 64], 3000, d_max=2000)
+    a = run_gpu(env, inp, chunks=[1000, 2000], path=1)
+    b = run_gpu(env, inp, chunks=[1000, 2000], path=1)
+    assert np.array_equal(a.view(np.float32), b.view(np.float32))            # run-to-run bitwise
+    perm = np.array([3, 6, 0, 5, 1, 4, 2])
+    c = run_gpu(env, inp.select_templates(perm), chunks=[1000, 2000], path=1)
+    assert np.array_equal(c.view(np.float32), a[perm].view(np.float32))      # rows permute bitwise
+
+
+def test_checkpoint_resume(env):
+    pkg, _, torch = env
+    inp = spiir_inputs.make_random_bank(31, [300, 77], 2000, d_max=500)
+    x = torch.from_numpy(inp.x).cuda()
+    full = run_gpu(env, inp, chunks=[1200, 800], path=1)
+    opt = pkg.SpiirOptions(path=1)                    # same kernel path as `full`, so the comparison is bitwise
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank:
+        snr = torch.empty((2, 2000), dtype=torch.complex64, device="cuda")
+        pkg.spiir_filter(bank.handle, x[:1200], snr[:, :1200])
+        y = torch.empty(inp.n_filters, dtype=torch.complex64, device="cuda")
+        hist = torch.empty(bank.max_delay, dtype=torch.float32, device="cuda")
+        pkg.spiir_bank_get_state(bank.handle, y, hist)
+        torch.cuda.synchronize()
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank2:
+        pkg.spiir_bank_set_state(bank2.handle, y, hist)
+        pkg.spiir_filter(bank2.handle, x[1200:], snr[:, 1200:])
+        torch.cuda.synchronize()
+    assert np.array_equal(snr.cpu().numpy().view(np.float32), full.view(np.float32))
+
+
+def test_reset_and_host_entry(env):
+    pkg, oracle, torch = env
+    inp = spiir_inputs.make_random_bank(41, [128, 512], 5000, d_max=900)
+    ref = oracle.run_inputs(inp)
+    check(run_gpu(env, inp, chunks=[2500, 2500], host=True), ref)
+    x = torch.from_numpy(inp.x).cuda()
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays) as bank:
+        first = bank.filter(x).cpu().numpy()
+        bank.reset()
+        second = bank.filter(x).cpu().numpy()
+    assert np.array_equal(first.view(np.float32), second.view(np.float32))
+    check(first, ref)
