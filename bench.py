@@ -1,0 +1,295 @@
+#!/usr/bin/env python
+"""bench.py -- SPIIR template-bank filter throughput on B200 (BASELINE.json metric and config).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: the streaming run of
+BASELINE.json:configs[3] (4096 templates x 1024 filters, 262 144 float32 samples fed as 16 chunks of 16 384
+with state carry), i.e. 16 spiir_filter calls = 1.0995e12 filter-samples.  Inputs are resident in HBM when the
+timed region starts (`value`); `e2e` repeats the measurement through spiir_filter_host with host buffers
+(H2D of every chunk and D2H of every SNR block inside the timed region).  Prints ONE JSON line.
+
+N > 1 (torchrun, one rank per GPU): templates are independent, so every rank filters
+its own seeded 4096-template bank -- no data-path collective -- and `value` is the total over ranks divided by
+the slowest rank's time ("scaling": "weak").
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores, on a bounded sample of the
+same workload; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import spiir_inputs  # noqa: E402
+
+METRIC = "SPIIR filter-samples/s (templates x filters x samples)"
+UNIT = "filter-samples/s"
+FLOPS_PER_FILTER_SAMPLE = 12          # complex*complex 6 + real*complex 2 + complex add 2 + sum 2
+N_SM, LANES, BOOST_HZ = 148, 128, 1.965e9   # B200: SMs x FP32 lanes x 2 flops x clocks.max.sm (MEASURED_PEAKS.json sm_max_mhz)
+FP32_PEAK_TFLOPS = N_SM * LANES * 2 * BOOST_HZ / 1e12    # 74.4 TFLOP/s, derivation in DESIGN.md section 7
+
+
+def workload_name(inp):
+    return (f"{inp.name}: {inp.n_templates} templates x {inp.n_filters // max(inp.n_templates, 1)} filters (mean), "
+            f"{inp.n_samples} samples, streaming in {inp.chunk}-sample chunks")
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (NVML; nvidia-smi semantics)."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _loop(self):
+        nv = self._nv
+        names = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "sw_power_cap": 0x4, "hw_power_brake_slowdown": 0x80}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def time_oracle(inp, n_templates: int, n_threads: int = 0):
+    """CPU oracle on the first n_templates templates of inp, all samples, streaming in inp.chunk chunks."""
+    import oracle
+    sub = inp.select_templates(np.arange(min(n_templates, inp.n_templates)))
+    oracle.build()
+    st = oracle.Stream(sub.offsets, sub.a1, sub.b0, sub.delays)
+    t0 = time.perf_counter()
+    for c0 in range(0, sub.n_samples, sub.chunk):
+        st.filter(sub.x[c0:c0 + sub.chunk], n_threads)
+    dt = time.perf_counter() - t0
+    st.close()
+    return sub.filter_samples / dt, dt, sub, oracle.max_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    inp = spiir_inputs.make_config(args.config)
+    n_tpl = args.ref_templates
+    for _ in range(args.warmup):
+        time_oracle(inp, max(1, n_tpl // 8))
+    rates, times = [], []
+    for _ in range(args.steps):
+        r, dt, sub, cores = time_oracle(inp, n_tpl)
+        rates.append(r)
+        times.append(dt)
+    total_fs = sub.filter_samples * args.steps
+    value = total_fs / sum(times)
+    sample = f"first {sub.n_templates} of {inp.n_templates} templates, all {inp.n_samples} samples, {inp.chunk}-sample chunks"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(inp), "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1602_05573_b200 as pkg
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the SPIIR library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    pkg.load_library()
+
+    # every rank filters its own seeded bank of the config's size (weak scaling, no exchange step)
+    inp = spiir_inputs.make_config(args.config)
+    if rank > 0:
+        rng = np.random.default_rng(spiir_inputs.SEED0 + 1000 * rank + args.config)
+        perm = rng.permutation(inp.n_templates)
+        inp = inp.select_templates(perm)               # same distributions, different bank per rank
+    N, L, T = inp.n_samples, inp.chunk, inp.n_templates
+    opt = pkg.SpiirOptions(path=args.path, filters_per_thread=args.filters_per_thread)
+    bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, local_rank, opt)
+    x = torch.from_numpy(inp.x).cuda()
+    keep_whole = (T * N * 8) <= args.max_snr_bytes
+    snr = torch.empty((T, N if keep_whole else L), dtype=torch.complex64, device="cuda")
+    stream = torch.cuda.current_stream()
+    n_calls = (N + L - 1) // L
+
+    def one_step(events=None):
+        bank.reset()
+        for i, c0 in enumerate(range(0, N, L)):
+            if events is not None:
+                events[i].record(stream)
+            n = min(L, N - c0)
+            out = snr[:, c0:c0 + n] if keep_whole else snr[:, :n]
+            pkg.spiir_filter(bank.handle, x[c0:c0 + n], out)
+        if events is not None:
+            events[n_calls].record(stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    barrier()
+    launches0 = pkg.spiir_kernel_launches()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(n_calls + 1)] for _ in range(args.steps)]
+    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        start.record(stream)
+        for s in range(args.steps):
+            one_step(ev[s])
+        stop.record(stream)
+        barrier()
+    launches = pkg.spiir_kernel_launches() - launches0
+    elapsed_ms = start.elapsed_time(stop)
+    call_ms = [ev[s][i].elapsed_time(ev[s][i + 1]) for s in range(args.steps) for i in range(n_calls)]
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    elapsed_ms_max = float(t.item())
+    fs_step = inp.filter_samples
+    value = world * fs_step * args.steps / (elapsed_ms_max * 1e-3)
+
+    # dominant kernel: spiir_filter_kernel, one launch per spiir_filter call (the call also enqueues one
+    # 64 KB device-to-device append of the chunk, < 0.1 % of the call)
+    fs_call = inp.n_filters * L
+    avg_call_s = float(np.mean(call_ms)) * 1e-3
+    achieved_tflops = FLOPS_PER_FILTER_SAMPLE * fs_call / avg_call_s / 1e12
+    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved_tflops / FP32_PEAK_TFLOPS, "traffic": args.ncu_traffic_bytes,
+                "kernel": "spiir_filter_kernel", "launch_ms": avg_call_s * 1e3,
+                "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1965 MHz (clocks.max.sm); no driver-measured FP32 peak exists",
+                "issue_slot_util": 8 * fs_call / avg_call_s / (N_SM * LANES * BOOST_HZ),
+                "hbm_write_gbs": 8.0 * T * L / avg_call_s / 1e9}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": elapsed_ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(inp), "path": bank.last_path,
+                       "l2": "each step writes %.2f GB of SNR and reads a %.0f MB bank: working set larger than the 126 MB L2"
+                             % (T * N * 8 / 1e9, inp.n_filters * 28 / 1e6),
+                       "snr_buffer": "whole [T][N]" if keep_whole else "per-chunk [T][L] reused"},
+            "pct_of_fp32_fma_peak": 100.0 * FLOPS_PER_FILTER_SAMPLE * value / world / (FP32_PEAK_TFLOPS * 1e12),
+            "gpu_launches": int(launches), "roofline": roofline, "clocks": clocks.summary()}
+
+    # ---- end to end through the public host-buffer entry (H2D + kernels + D2H inside the timed region)
+    if not args.no_e2e:
+        xh = torch.from_numpy(inp.x).pin_memory()
+        outh = torch.empty((T, L), dtype=torch.complex64).pin_memory()
+        xh_np, outh_np = xh.numpy(), outh.numpy()
+
+        def e2e_step():
+            bank.reset()
+            for c0 in range(0, N, L):
+                n = min(L, N - c0)
+                pkg.spiir_filter_host(bank.handle, xh_np[c0:c0 + n], outh_np[:, :n])
+
+        e2e_step()
+        barrier()
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        line["e2e"] = {"value": world * fs_step * e2e_steps / float(tt.item()), "unit": UNIT,
+                       "h2d_bytes_per_step": int(N * 4), "d2h_bytes_per_step": int(T * N * 8),
+                       "steps": e2e_steps, "api": "spiir_filter_host (pinned host buffers)"}
+
+    # ---- the CPU oracle beside it (rank 0, N = 1 only): a reported baseline, not the target
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r, dt, sub, cores = time_oracle(inp, args.cpu_templates)
+        line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+                                "sample": f"first {sub.n_templates} of {T} templates, all {N} samples, {L}-sample chunks"}
+    bank.close()
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json:configs (3 = headline)")
+    ap.add_argument("--path", type=int, default=0, help="SPIIR_PATH_* override (0 auto)")
+    ap.add_argument("--filters-per-thread", type=int, default=0)
+    ap.add_argument("--max-snr-bytes", type=float, default=20e9, help="keep the whole [T][N] SNR if it fits")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-templates", type=int, default=96, help="templates of the bounded oracle sample")
+    ap.add_argument("--ref-templates", type=int, default=32, help="templates per step of --impl reference")
+    ap.add_argument("--ncu-traffic-bytes", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
