@@ -39,8 +39,6 @@ int fail(int code, const char* fmt, ...)
                         cudaGetErrorString(e_));                                                  \
     } while (0)
 
-constexpr size_t kPartBytes = 2ull * kWarpsPerCta * kTS * sizeof(u64);
-
 template <typename T>
 cudaError_t upload(T** dst, const std::vector<T>& v)
 {
@@ -56,7 +54,8 @@ cudaError_t upload(T** dst, const std::vector<T>& v)
 
 struct spiir_bank {
     int device = 0;
-    int F = 8;
+    int F = 8, W = 16;
+    bool configured[2] = {false, false};
     int64_t T = 0, K = 0, D = 0, n_slots = 0, n_tiles = 0;
     int32_t n_items = 0;
     double avg_conflict_degree = 0.0;
@@ -140,59 +139,60 @@ int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
     return SPIIR_OK;
 }
 
-// allow the kernel to use all opt-in shared memory (once per instantiation and device)
-template <int F, bool G>
-int configure_kernel(int device, size_t smem_optin)
+// The compiled (F, W) register/warp blockings of the filter kernel: F filters per thread, W warps per CTA.
+// W is chosen so that the register file of an SM is full with one resident CTA (the shared-memory window of
+// a 16 384-sample chunk behind a 16 383-sample history allows only one).
+const void* select_kernel(int F, int W, bool g)
 {
-    static std::atomic<uint64_t> done_mask{0};
-    const uint64_t bit = 1ull << (device & 63);
-    if (done_mask.load(std::memory_order_acquire) & bit) return SPIIR_OK;
-    CU_TRY(cudaFuncSetAttribute(spiir_filter_kernel<F, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_optin));
-    done_mask.fetch_or(bit, std::memory_order_release);
+#define SPIIR_VARIANT(F_, W_)                                                                            \
+    if (F == F_ && W == W_)                                                                              \
+        return g ? (const void*)spiir_filter_kernel<F_, W_, true> : (const void*)spiir_filter_kernel<F_, W_, false>;
+    SPIIR_VARIANT(16, 8)
+    SPIIR_VARIANT(8, 8)
+    SPIIR_VARIANT(8, 16)
+    SPIIR_VARIANT(4, 16)
+    SPIIR_VARIANT(4, 32)
+    SPIIR_VARIANT(2, 32)
+#undef SPIIR_VARIANT
+    return nullptr;
+}
+
+bool valid_blocking(int F, int W) { return select_kernel(F, W, false) != nullptr; }
+
+int default_warps(int F) { return F >= 16 ? 8 : (F == 8 ? 16 : 32); }
+
+size_t part_bytes(const spiir_bank* bk) { return 2ull * bk->W * kTS * sizeof(u64); }
+
+// allow the kernel to use all opt-in shared memory (once per variant and bank)
+int configure_kernel(spiir_bank* bk, bool g, const void** fn)
+{
+    *fn = select_kernel(bk->F, bk->W, g);
+    if (!*fn) return fail(SPIIR_EINVAL, "unsupported blocking F=%d W=%d", bk->F, bk->W);
+    if (!bk->configured[g]) {
+        CU_TRY(cudaFuncSetAttribute(*fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bk->smem_optin));
+        bk->configured[g] = true;
+    }
     return SPIIR_OK;
 }
 
-template <int F, bool G>
-int launch_one(const spiir_bank* bk, const FilterParams& p, dim3 grid, size_t smem, cudaStream_t st)
+int launch_filter(spiir_bank* bk, bool g, const FilterParams& p, dim3 grid, size_t smem, cudaStream_t st)
 {
-    int rc = configure_kernel<F, G>(bk->device, bk->smem_optin);
+    const void* fn = nullptr;
+    int rc = configure_kernel(bk, g, &fn);
     if (rc) return rc;
-    spiir_filter_kernel<F, G><<<grid, kThreads, smem, st>>>(p);
+    void* args[] = {(void*)&p};
+    CU_TRY(cudaLaunchKernel(fn, grid, dim3((unsigned)(kWarp * bk->W), 1, 1), args, smem, st));
     g_launches.fetch_add(1, std::memory_order_relaxed);
-    CU_TRY(cudaGetLastError());
     return SPIIR_OK;
 }
 
-template <bool G>
-int launch_F(const spiir_bank* bk, const FilterParams& p, dim3 grid, size_t smem, cudaStream_t st)
+int occupancy(spiir_bank* bk, bool g, size_t smem, int* occ)
 {
-    switch (bk->F) {
-        case 2: return launch_one<2, G>(bk, p, grid, smem, st);
-        case 4: return launch_one<4, G>(bk, p, grid, smem, st);
-        case 8: return launch_one<8, G>(bk, p, grid, smem, st);
-        case 16: return launch_one<16, G>(bk, p, grid, smem, st);
-    }
-    return fail(SPIIR_EINVAL, "unsupported filters_per_thread %d", bk->F);
-}
-
-template <int F, bool G>
-int occupancy_one(const spiir_bank* bk, size_t smem, int* occ)
-{
-    int rc = configure_kernel<F, G>(bk->device, bk->smem_optin);
+    const void* fn = nullptr;
+    int rc = configure_kernel(bk, g, &fn);
     if (rc) return rc;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, spiir_filter_kernel<F, G>, kThreads, smem));
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, fn, kWarp * bk->W, smem));
     return SPIIR_OK;
-}
-
-int occupancy(const spiir_bank* bk, bool g, size_t smem, int* occ)
-{
-    switch (bk->F) {
-        case 2: return g ? occupancy_one<2, true>(bk, smem, occ) : occupancy_one<2, false>(bk, smem, occ);
-        case 4: return g ? occupancy_one<4, true>(bk, smem, occ) : occupancy_one<4, false>(bk, smem, occ);
-        case 8: return g ? occupancy_one<8, true>(bk, smem, occ) : occupancy_one<8, false>(bk, smem, occ);
-        case 16: return g ? occupancy_one<16, true>(bk, smem, occ) : occupancy_one<16, false>(bk, smem, occ);
-    }
-    return fail(SPIIR_EINVAL, "unsupported filters_per_thread %d", bk->F);
 }
 
 int cached_occupancy(spiir_bank* bk, bool g, size_t smem, int* occ)
@@ -218,6 +218,7 @@ FilterParams base_params(const spiir_bank* bk)
 int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st)
 {
     const size_t smem_cap = bk->smem_optin;
+    const size_t kPartBytes = part_bytes(bk);
     const int64_t max_win = ((int64_t)smem_cap - (int64_t)kPartBytes) / 4 - 8;   // floats
     const bool gmem = (w0 + kTS > max_win);   // history alone does not fit: read x through L1/L2
     int path = bk->opt.path;
@@ -246,7 +247,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
             if (rc) return rc;
             if (occ < 1) return fail(SPIIR_ECUDA, "filter kernel does not fit on an SM (smem %zu)", smem);
             dim3 grid((unsigned)std::min<int64_t>(bk->n_items, (int64_t)bk->n_sm * occ), 1, 1);
-            rc = gmem ? launch_F<true>(bk, p, grid, smem, st) : launch_F<false>(bk, p, grid, smem, st);
+            rc = launch_filter(bk, gmem, p, grid, smem, st);
             if (rc) return rc;
         }
         return SPIIR_OK;
@@ -278,7 +279,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
         p.xwin = xwin; p.w0 = w0; p.n = (n_seg - 1) * seg_len; p.seg_len = seg_len;
         p.snr = nullptr; p.ld = 0;
         dim3 grid(gx, (unsigned)(n_seg - 1), 1);
-        rc = gmem ? launch_F<true>(bk, p, grid, smem, st) : launch_F<false>(bk, p, grid, smem, st);
+        rc = launch_filter(bk, gmem, p, grid, smem, st);
         if (rc) return rc;
     }
     {
@@ -297,7 +298,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
         p.xwin = xwin; p.w0 = w0; p.n = n; p.seg_len = seg_len;
         p.snr = snr; p.ld = ld;
         dim3 grid(gx, (unsigned)n_seg, 1);
-        rc = gmem ? launch_F<true>(bk, p, grid, smem, st) : launch_F<false>(bk, p, grid, smem, st);
+        rc = launch_filter(bk, gmem, p, grid, smem, st);
         if (rc) return rc;
     }
     return SPIIR_OK;
@@ -357,6 +358,8 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
             o.filters_per_thread != 8 && o.filters_per_thread != 16)
             return fail(SPIIR_EINVAL, "filters_per_thread must be 0, 2, 4, 8 or 16");
         if (o.scan_segments < 0) return fail(SPIIR_EINVAL, "scan_segments must be >= 0");
+        if (o.warps_per_cta != 0 && o.warps_per_cta != 8 && o.warps_per_cta != 16 && o.warps_per_cta != 32)
+            return fail(SPIIR_EINVAL, "warps_per_cta must be 0, 8, 16 or 32");
     }
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0)
@@ -370,9 +373,15 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->opt = o;
     bk->T = T; bk->K = K; bk->D = D;
     bk->F = choose_F(T, off, o.filters_per_thread);
+    bk->W = o.warps_per_cta ? o.warps_per_cta : default_warps(bk->F);
+    if (!valid_blocking(bk->F, bk->W)) {
+        const int F = bk->F, W = bk->W;
+        free_bank(bk);
+        return fail(SPIIR_EINVAL, "unsupported blocking: filters_per_thread %d with warps_per_cta %d", F, W);
+    }
     HostLayout L;
     try {
-        L = build_layout(T, off, a1, b0, delays, bk->F);
+        L = build_layout(T, off, a1, b0, delays, bk->F, bk->W);
     } catch (const std::bad_alloc&) {
         free_bank(bk);
         return fail(SPIIR_ENOMEM, "out of host memory building the bank layout");

@@ -27,7 +27,6 @@ typedef unsigned long long u64;
 
 constexpr int kTT = 8;        // samples per register tile
 constexpr int kTS = 64;       // samples per super tile (cross-warp combine + output granularity)
-constexpr int kThreads = kWarp * kWarpsPerCta;
 
 __device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
 __device__ __forceinline__ u64 fmul2(u64 a, u64 b) { u64 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
@@ -116,9 +115,10 @@ __device__ __forceinline__ u64 warp_reduce_tile(u64 (&S)[kTT], int lane)
 
 // Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
 // Dynamic shared memory: [xwin window floats][2 * W * kTS complex partial sums].
-template <int F, bool GMEM_X>
-__global__ void __launch_bounds__(kThreads) spiir_filter_kernel(const FilterParams p)
+template <int F, int W, bool GMEM_X>
+__global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterParams p)
 {
+    constexpr int kThreads = kWarp * W;
     extern __shared__ __align__(16) float smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int seg = blockIdx.y;
@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(kThreads) spiir_filter_kernel(const FilterPara
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
         const int r0 = p.item_round0[item], r1 = p.item_round0[item + 1];
         for (int r = r0; r < r1; ++r) {
-            const WarpWork ww = p.work[r * kWarpsPerCta + warp];
+            const WarpWork ww = p.work[r * W + warp];
             const bool active = ww.tile >= 0;
             float ar[F];
             u64 AI[F], B[F], Y[F];
@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(kThreads) spiir_filter_kernel(const FilterPara
             for (int64_t st = 0; st < nseg; st += kTS, buf ^= 1) {
                 const int ns = (int)min((int64_t)kTS, nseg - st);
                 if (active) {
-                    u64* mypart = part64 + ((size_t)buf * kWarpsPerCta + warp) * kTS;
+                    u64* mypart = part64 + ((size_t)buf * W + warp) * kTS;
 #pragma unroll 1
                     for (int tt = 0; tt < ns; tt += kTT) {
                         u64 S[kTT];
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(kThreads) spiir_filter_kernel(const FilterPara
                     __syncthreads();
                     if (active) {
                         // warps of one template share its ns samples; fixed summation order over warps
-                        const u64* pb = part64 + (size_t)buf * kWarpsPerCta * kTS;
+                        const u64* pb = part64 + (size_t)buf * W * kTS;
                         for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
                             u64 acc = pb[(size_t)ww.first * kTS + s];
                             for (int w = 1; w < ww.count; ++w) acc = fadd2(acc, pb[(size_t)(ww.first + w) * kTS + s]);

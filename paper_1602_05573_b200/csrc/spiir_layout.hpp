@@ -20,7 +20,6 @@
 namespace spiir {
 
 constexpr int kWarp = 32;
-constexpr int kWarpsPerCta = 8;   // W: warps of one CTA = warp tiles processed side by side
 
 struct WarpWork {        // what one warp does in one round of one CTA item
     int32_t tile;        // warp tile index into the slot arrays, -1 = idle
@@ -31,6 +30,7 @@ struct WarpWork {        // what one warp does in one round of one CTA item
 
 struct HostLayout {
     int F = 0;                          // register slots (filters) per thread
+    int W = 0;                          // warps of one CTA = warp tiles processed side by side
     int64_t n_tiles = 0;                // warp tiles
     int64_t n_slots = 0;                // n_tiles * F * 32
     std::vector<float> ar;              // [n_slots] Re a1
@@ -39,9 +39,9 @@ struct HostLayout {
     std::vector<int32_t> dly;           // [n_slots]
     std::vector<int64_t> slot_of_filter;  // [K] caller's filter index -> slot
     std::vector<int64_t> tile_begin;    // [T+1] first tile of each template
-    // work list: items (one CTA at a time), each with >= 1 rounds of kWarpsPerCta warp entries
+    // work list: items (one CTA at a time), each with >= 1 rounds of W warp entries
     std::vector<int32_t> item_round0;   // [n_items+1] first round of each item
-    std::vector<WarpWork> work;         // [n_rounds * kWarpsPerCta]
+    std::vector<WarpWork> work;         // [n_rounds * W]
     double avg_conflict_degree = 0.0;   // mean over groups of max residue multiplicity (diagnostic)
 };
 
@@ -105,10 +105,11 @@ inline void deal_groups(const int32_t* d, const std::vector<int64_t>& order, int
 }
 
 inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, const float* b0,
-                               const int32_t* d, int F)
+                               const int32_t* d, int F, int W)
 {
     HostLayout L;
     L.F = F;
+    L.W = W;
     const int64_t K = off[T];
     L.tile_begin.resize((size_t)T + 1);
     int64_t tiles = 0;
@@ -165,7 +166,6 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
 
     // Work list.  Templates with <= W tiles share an item round with their neighbours (greedy, in bank
     // order); a template with more tiles gets an item of its own with several accumulate rounds.
-    const int W = kWarpsPerCta;
     L.item_round0.push_back(0);
     std::vector<WarpWork> cur;
     auto flush = [&]() {
