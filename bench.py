@@ -158,7 +158,8 @@ def run_ours(args):
         perm = rng.permutation(inp.n_templates)
         inp = inp.select_templates(perm)               # same distributions, different bank per rank
     N, L, T = inp.n_samples, inp.chunk, inp.n_templates
-    opt = pkg.SpiirOptions(path=args.path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta)
+    opt = pkg.SpiirOptions(path=args.path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta,
+                           window_copies=args.window_copies)
     bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, local_rank, opt)
     x = torch.from_numpy(inp.x).cuda()
     keep_whole = (T * N * 8) <= args.max_snr_bytes
@@ -278,6 +279,7 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="SPIIR_PATH_* override (0 auto)")
     ap.add_argument("--filters-per-thread", type=int, default=0)
     ap.add_argument("--warps-per-cta", type=int, default=0)
+    ap.add_argument("--window-copies", type=int, default=0)
     ap.add_argument("--max-snr-bytes", type=float, default=20e9, help="keep the whole [T][N] SNR if it fits")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")

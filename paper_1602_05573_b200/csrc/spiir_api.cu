@@ -54,7 +54,8 @@ cudaError_t upload(T** dst, const std::vector<T>& v)
 
 struct spiir_bank {
     int device = 0;
-    int F = 8, W = 16;
+    int F = 8, W = 16, NC = 1;
+    bool gmem_only = false;          // the history alone exceeds shared memory: x is read through L1/L2
     bool configured[2] = {false, false};
     int64_t T = 0, K = 0, D = 0, n_slots = 0, n_tiles = 0;
     int32_t n_items = 0;
@@ -142,11 +143,15 @@ int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
 // The compiled (F, W) register/warp blockings of the filter kernel: F filters per thread, W warps per CTA.
 // W is chosen so that the register file of an SM is full with one resident CTA (the shared-memory window of
 // a 16 384-sample chunk behind a 16 383-sample history allows only one).
-const void* select_kernel(int F, int W, bool g)
+const void* select_kernel(int F, int W, int NC, bool g)
 {
-#define SPIIR_VARIANT(F_, W_)                                                                            \
-    if (F == F_ && W == W_)                                                                              \
-        return g ? (const void*)spiir_filter_kernel<F_, W_, true> : (const void*)spiir_filter_kernel<F_, W_, false>;
+#define SPIIR_VARIANT(F_, W_)                                                                  \
+    if (F == F_ && W == W_) {                                                                  \
+        if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true>;                       \
+        if (NC == 4) return (const void*)spiir_filter_kernel<F_, W_, 4, false>;                \
+        if (NC == 2) return (const void*)spiir_filter_kernel<F_, W_, 2, false>;                \
+        return (const void*)spiir_filter_kernel<F_, W_, 1, false>;                             \
+    }
     SPIIR_VARIANT(16, 8)
     SPIIR_VARIANT(8, 8)
     SPIIR_VARIANT(8, 16)
@@ -157,16 +162,17 @@ const void* select_kernel(int F, int W, bool g)
     return nullptr;
 }
 
-bool valid_blocking(int F, int W) { return select_kernel(F, W, false) != nullptr; }
+bool valid_blocking(int F, int W) { return select_kernel(F, W, 1, false) != nullptr; }
 
 int default_warps(int F) { return F >= 16 ? 8 : (F == 8 ? 16 : 32); }
 
-size_t part_bytes(const spiir_bank* bk) { return 2ull * bk->W * kTS * sizeof(u64); }
+// shared memory besides the window copies
+size_t fixed_smem(int W) { return filter_smem_bytes(W, 1, 0, true, nullptr); }
 
 // allow the kernel to use all opt-in shared memory (once per variant and bank)
 int configure_kernel(spiir_bank* bk, bool g, const void** fn)
 {
-    *fn = select_kernel(bk->F, bk->W, g);
+    *fn = select_kernel(bk->F, bk->W, bk->NC, g);
     if (!*fn) return fail(SPIIR_EINVAL, "unsupported blocking F=%d W=%d", bk->F, bk->W);
     if (!bk->configured[g]) {
         CU_TRY(cudaFuncSetAttribute(*fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bk->smem_optin));
@@ -218,9 +224,9 @@ FilterParams base_params(const spiir_bank* bk)
 int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st)
 {
     const size_t smem_cap = bk->smem_optin;
-    const size_t kPartBytes = part_bytes(bk);
-    const int64_t max_win = ((int64_t)smem_cap - (int64_t)kPartBytes) / 4 - 8;   // floats
-    const bool gmem = (w0 + kTS > max_win);   // history alone does not fit: read x through L1/L2
+    // window floats per copy that fit beside the reduction buffers (a copy is padded by up to 47 floats)
+    const int64_t max_win = ((int64_t)smem_cap - (int64_t)fixed_smem(bk->W)) / (4 * bk->NC) - 48;
+    const bool gmem = bk->gmem_only;          // history alone does not fit: read x through L1/L2
     int path = bk->opt.path;
     // ---- how much time-parallelism is needed to fill the machine?
     int64_t n_seg = 1;
@@ -234,14 +240,19 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     if (n_seg <= 1) {
         // ------------------------------------------------ sequential-in-time path
         bk->last_path = (path == SPIIR_PATH_STREAM) ? SPIIR_PATH_STREAM : SPIIR_PATH_THROUGHPUT;
-        const int64_t sub = gmem ? n : std::max<int64_t>(kTS, (max_win - w0) / kTS * kTS);
+        int64_t sub = n;
+        if (!gmem) {
+            const int64_t sub_max = std::max<int64_t>(kTS, (max_win - w0) / kTS * kTS);
+            const int64_t n_launch = (n + sub_max - 1) / sub_max;                 // balanced sub-launches
+            sub = std::min(sub_max, round_up((n + n_launch - 1) / n_launch, kTS));
+        }
         for (int64_t off = 0; off < n; off += sub) {
             const int64_t ns = std::min(sub, n - off);
             FilterParams p = base_params(bk);
             p.y_in = bk->y; p.y_out = bk->y; p.y_in_stride = 0; p.y_out_stride = 0; p.store_last_only = 1;
             p.xwin = xwin + off; p.w0 = w0; p.n = ns; p.seg_len = ns;
             p.snr = snr + 2 * off; p.ld = ld;
-            const size_t smem = gmem ? kPartBytes : (size_t)round_up(w0 + ns, 4) * 4 + kPartBytes;
+            const size_t smem = filter_smem_bytes(bk->W, bk->NC, w0 + ns, gmem, nullptr);
             int occ = 1;
             int rc = cached_occupancy(bk, gmem, smem, &occ);
             if (rc) return rc;
@@ -266,7 +277,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
         CU_TRY(cudaMalloc((void**)&bk->cbuf, bytes));
         bk->scan_cap_seg = n_seg;
     }
-    const size_t smem = gmem ? kPartBytes : (size_t)round_up(w0 + seg_len, 4) * 4 + kPartBytes;
+    const size_t smem = filter_smem_bytes(bk->W, bk->NC, w0 + seg_len, gmem, nullptr);
     int occ = 1;
     int rc = cached_occupancy(bk, gmem, smem, &occ);
     if (rc) return rc;
@@ -360,6 +371,8 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         if (o.scan_segments < 0) return fail(SPIIR_EINVAL, "scan_segments must be >= 0");
         if (o.warps_per_cta != 0 && o.warps_per_cta != 8 && o.warps_per_cta != 16 && o.warps_per_cta != 32)
             return fail(SPIIR_EINVAL, "warps_per_cta must be 0, 8, 16 or 32");
+        if (o.window_copies != 0 && o.window_copies != 1 && o.window_copies != 2 && o.window_copies != 4)
+            return fail(SPIIR_EINVAL, "window_copies must be 0, 1, 2 or 4");
     }
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0)
@@ -379,9 +392,31 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         free_bank(bk);
         return fail(SPIIR_EINVAL, "unsupported blocking: filters_per_thread %d with warps_per_cta %d", F, W);
     }
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) {
+        free_bank(bk);
+        return fail(SPIIR_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
+    }
+    bk->n_sm = prop.multiProcessorCount;
+    bk->smem_optin = prop.sharedMemPerBlockOptin;
+    // Window copies: as many (4, 2, 1 = LDS.128/.64/.32 per filter) as leave room for >= kMinSub samples per
+    // launch behind the history; none at all (global-memory reads) if not even one copy of the history fits.
+    {
+        const int64_t room = (int64_t)bk->smem_optin - (int64_t)fixed_smem(bk->W);
+        const int64_t hist = round_up(D, 4) + 4 + 48;
+        const int64_t kMinSub = 2048;
+        bk->NC = 1;
+        for (int nc : {4, 2})
+            if ((hist + kMinSub) * 4 * nc <= room) { bk->NC = nc; break; }
+        if (o.window_copies == 1 || o.window_copies == 2 || o.window_copies == 4)
+            if ((hist + kTS) * 4 * o.window_copies <= room) bk->NC = o.window_copies;
+        bk->gmem_only = (hist + kTS) * 4 > room;
+        if (bk->gmem_only) bk->NC = 1;
+    }
     HostLayout L;
     try {
-        L = build_layout(T, off, a1, b0, delays, bk->F, bk->W);
+        L = build_layout(T, off, a1, b0, delays, bk->F, bk->W, bk->NC);
     } catch (const std::bad_alloc&) {
         free_bank(bk);
         return fail(SPIIR_ENOMEM, "out of host memory building the bank layout");
@@ -390,12 +425,6 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->n_tiles = L.n_tiles;
     bk->n_items = (int32_t)(L.item_round0.size() - 1);
     bk->avg_conflict_degree = L.avg_conflict_degree;
-    cudaDeviceProp prop;
-    cudaError_t e = cudaGetDeviceProperties(&prop, device);
-    if (e == cudaSuccess) {
-        bk->n_sm = prop.multiProcessorCount;
-        bk->smem_optin = prop.sharedMemPerBlockOptin;
-    }
     if (e == cudaSuccess) e = upload(&bk->ar, L.ar);
     if (e == cudaSuccess) e = upload(&bk->ai2, L.ai2);
     if (e == cudaSuccess) e = upload(&bk->b, L.b);

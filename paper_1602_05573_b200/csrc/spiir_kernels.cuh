@@ -63,61 +63,105 @@ struct FilterParams {
 };
 
 // One register tile: advance F filters by NV <= 8 samples, S[j] = sum over the thread's filters.
-template <int F, bool FULL>
+// The delayed input comes from NC shifted copies of the window (copy c holds win[i + c]), so that every
+// filter reads NC consecutive samples with one aligned LDS.32 / LDS.64 / LDS.128 (xo[f] already points
+// into the copy that makes its loads aligned).
+template <int F, int NC, bool FULL>
 __device__ __forceinline__ void tile_step(const float* __restrict__ xs, const int (&xo)[F], const float (&ar)[F],
                                           const u64 (&AI)[F], const u64 (&B)[F], u64 (&Y)[F], u64 (&S)[kTT],
                                           int tb, int nv)
 {
 #pragma unroll
-    for (int j = 0; j < kTT; ++j) {
-        if (FULL || j < nv) {
+    for (int jb = 0; jb < kTT; jb += NC) {
+        float xv[F][NC];
 #pragma unroll
-            for (int f = 0; f < F; ++f) {
-                const float x = xs[xo[f] + tb + j];
-                u64 t = fmul2(B[f], pack2(x, x));
-                float yr, yi;
-                unpack2(Y[f], yr, yi);
-                t = ffma2(AI[f], pack2(yi, yr), t);
-                Y[f] = ffma2(pack2(ar[f], ar[f]), Y[f], t);
-                S[j] = (f == 0) ? Y[f] : fadd2(S[j], Y[f]);
+        for (int f = 0; f < F; ++f) {
+            const float* px = xs + xo[f] + tb + jb;
+            if (NC == 4) {
+                const float4 v = *reinterpret_cast<const float4*>(px);
+                xv[f][0] = v.x; xv[f][1] = v.y; xv[f][NC > 2 ? 2 : 0] = v.z; xv[f][NC > 2 ? 3 : 0] = v.w;
+            } else if (NC == 2) {
+                const float2 v = *reinterpret_cast<const float2*>(px);
+                xv[f][0] = v.x; xv[f][NC > 1 ? 1 : 0] = v.y;
+            } else {
+                xv[f][0] = *px;
             }
-        } else {
-            S[j] = 0ull;
+        }
+#pragma unroll
+        for (int jj = 0; jj < NC; ++jj) {
+            const int j = jb + jj;
+            if (FULL || j < nv) {
+#pragma unroll
+                for (int f = 0; f < F; ++f) {
+                    const float x = xv[f][jj];
+                    u64 t = fmul2(B[f], pack2(x, x));
+                    float yr, yi;
+                    unpack2(Y[f], yr, yi);
+                    t = ffma2(AI[f], pack2(yi, yr), t);
+                    Y[f] = ffma2(pack2(ar[f], ar[f]), Y[f], t);
+                    S[j] = (f == 0) ? Y[f] : fadd2(S[j], Y[f]);
+                }
+            } else {
+                S[j] = 0ull;
+            }
         }
     }
 }
 
-// Transposing butterfly: on return every lane holds the warp-wide sum of sample bitrev3(lane & 7).
-__device__ __forceinline__ u64 warp_reduce_tile(u64 (&S)[kTT], int lane)
+// Cross-lane sum of a register tile through a per-warp shared-memory transpose.  Lane l writes its 8
+// partial sums as row l (4 x STS.128, rows padded to 10 u64 = 80 B so that a quarter warp hits all bank
+// groups); then lane (g = l >> 3, j = l & 7) adds sample j of the 8 rows of lane group g (8 x LDS.64,
+// rows visited in an order that keeps the two groups of a half warp on different banks) and two
+// shuffle steps add the 4 groups.  Fixed order, no atomics.  Lanes 0..7 return the warp sum of sample
+// `lane`.  Costs ~30 issue slots per tile against ~64 for a shuffle-only transposing butterfly.
+constexpr int kTrRow = 10;                      // u64 per scratch row
+constexpr int kTrWarp = kWarp * kTrRow;         // u64 per warp
+
+__device__ __forceinline__ u64 warp_reduce_tile(u64 (&S)[kTT], u64* __restrict__ tr, int lane)
 {
     const unsigned full = 0xffffffffu;
-    u64 R[4], Q[2];
-    const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4;
+    ulonglong2* row = reinterpret_cast<ulonglong2*>(tr + lane * kTrRow);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const u64 send = b0 ? S[i] : S[i + 4];
-        const u64 keep = b0 ? S[i + 4] : S[i];
-        R[i] = fadd2(keep, __shfl_xor_sync(full, send, 1));
-    }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const u64 send = b1 ? R[i] : R[i + 2];
-        const u64 keep = b1 ? R[i + 2] : R[i];
-        Q[i] = fadd2(keep, __shfl_xor_sync(full, send, 2));
-    }
-    const u64 send = b2 ? Q[0] : Q[1];
-    const u64 keep = b2 ? Q[1] : Q[0];
-    u64 P = fadd2(keep, __shfl_xor_sync(full, send, 4));
+    for (int c = 0; c < kTT / 2; ++c) row[c] = make_ulonglong2(S[2 * c], S[2 * c + 1]);
+    __syncwarp();
+    const int g = lane >> 3, j = lane & 7, b = g & 1;
+    const u64* ra = tr + (g * 8 + 4 * b) * kTrRow + j;
+    const u64* rb = tr + (g * 8 + 4 * (1 - b)) * kTrRow + j;
+    const u64 s0 = fadd2(ra[0], ra[kTrRow]), s1 = fadd2(ra[2 * kTrRow], ra[3 * kTrRow]);
+    const u64 s2 = fadd2(rb[0], rb[kTrRow]), s3 = fadd2(rb[2 * kTrRow], rb[3 * kTrRow]);
+    // (rows g*8..g*8+3) + (rows g*8+4..g*8+7): IEEE addition commutes, so the half a lane read first is immaterial
+    u64 P = fadd2(fadd2(s0, s1), fadd2(s2, s3));
+    __syncwarp();                               // rows may be overwritten by the next tile
     P = fadd2(P, __shfl_xor_sync(full, P, 8));
     P = fadd2(P, __shfl_xor_sync(full, P, 16));
     return P;
 }
 
+// Barrier over the warps of one template in the current round (they sit on different SM sub-partitions;
+// templates drift apart freely, so one template's reduction overlaps the others' arithmetic).  Groups of
+// >= 2 warps start at least 2 warps apart, so first/2 is a unique hardware barrier id in 0..15.
+__device__ __forceinline__ void group_barrier(const WarpWork& ww)
+{
+    if (ww.count > 1) asm volatile("bar.sync %0, %1;" ::"r"(ww.first >> 1), "r"(ww.count * kWarp) : "memory");
+    else __syncwarp();
+}
+
+// Shared memory of the filter kernel, in this order:
+//   NC window copies of `cstride` floats each (absent when GMEM_X), W transpose scratches, 2 x W x kTS partial sums
+__host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_len, bool gmem_x, int64_t* cstride_out)
+{
+    // copy stride = 0 mod 32 floats: every copy starts on bank 0, as the lane dealing assumes
+    const int64_t cstride = gmem_x ? 0 : ((win_len + 16 + 31) / 32 * 32);
+    if (cstride_out) *cstride_out = cstride;
+    return (size_t)(gmem_x ? 0 : NC * cstride) * sizeof(float) + (size_t)W * kTrWarp * sizeof(u64) +
+           2ull * W * kTS * sizeof(u64);
+}
+
 // Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
-// Dynamic shared memory: [xwin window floats][2 * W * kTS complex partial sums].
-template <int F, int W, bool GMEM_X>
+template <int F, int W, int NC, bool GMEM_X>
 __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterParams p)
 {
+    static_assert(!GMEM_X || NC == 1, "the global-memory window variant reads scalars");
     constexpr int kThreads = kWarp * W;
     extern __shared__ __align__(16) float smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -126,23 +170,36 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
     const int64_t nseg = min(p.seg_len, p.n - t0);
     if (nseg <= 0) return;
 
-    // ---- stage the input window [t0 - w0, t0 + nseg) into shared memory
-    const int64_t win0 = t0;                                  // index in xwin of the window start (mult of 4)
+    // ---- stage the input window [t0 - w0, t0 + nseg) into shared memory, NC times (copy c shifted by c)
     const int win_len = p.w0 + (int)nseg;
-    const int win_pad = (win_len + 3) & ~3;
+    int64_t cstride;
+    filter_smem_bytes(W, NC, win_len, GMEM_X, &cstride);
     const float* xs;
-    float* part;
     if (GMEM_X) {
-        xs = p.xwin + win0;
-        part = smem;
+        xs = p.xwin + t0;
     } else {
-        const float4* src = reinterpret_cast<const float4*>(p.xwin + win0);
-        float4* dst = reinterpret_cast<float4*>(smem);
-        for (int i = tid; i < win_pad / 4; i += kThreads) dst[i] = src[i];
+        const float4* src = reinterpret_cast<const float4*>(p.xwin + t0);   // t0 and xwin are 16-byte aligned
+        const int n4 = (int)(cstride / 4);
+        const int v4 = (win_len + 3) / 4;                                    // float4s that hold valid samples
+        for (int i = tid; i < n4; i += kThreads) {
+            const float4 v = i < v4 ? src[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+            reinterpret_cast<float4*>(smem)[i] = v;
+            if (NC > 1) {
+                const float e[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int c = 1; c < NC; ++c) {
+                    float* dst = smem + (int64_t)c * cstride + 4 * i - c;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (4 * i + q - c >= 0) dst[q] = e[q];
+                }
+            }
+        }
         xs = smem;
-        part = smem + win_pad;
     }
-    u64* part64 = reinterpret_cast<u64*>(part);               // [2][W][kTS]
+    u64* trbuf = reinterpret_cast<u64*>(smem + (GMEM_X ? 0 : NC * cstride));   // [W][kTrWarp]
+    u64* part64 = trbuf + (size_t)W * kTrWarp;                                 // [2][W][kTS]
+    u64* mytr = trbuf + (size_t)warp * kTrWarp;
     __syncthreads();
 
     const bool last_seg = (t0 + nseg >= p.n);
@@ -162,7 +219,9 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
                     AI[f] = ld_pair(p.ai2 + 2 * s);
                     B[f] = ld_pair(p.b + 2 * s);
                     Y[f] = p.y_in ? ld_pair(p.y_in + (int64_t)seg * p.y_in_stride + 2 * s) : 0ull;
-                    xo[f] = p.w0 - p.dly[s];
+                    const int p0 = p.w0 - p.dly[s];            // window index of this filter's first input
+                    const int c = p0 & (NC - 1);               // the copy in which p0 is aligned
+                    xo[f] = (int)(c * cstride) + p0 - c;
                 } else {
                     ar[f] = 0.f; AI[f] = 0ull; B[f] = 0ull; Y[f] = 0ull; xo[f] = 0;
                 }
@@ -177,20 +236,17 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
                     for (int tt = 0; tt < ns; tt += kTT) {
                         u64 S[kTT];
                         const int nv = ns - tt;
-                        if (nv >= kTT) tile_step<F, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
-                        else tile_step<F, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
+                        if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
+                        else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
                         if (p.snr) {
-                            const u64 P = warp_reduce_tile(S, lane);
-                            if (lane < kTT) {
-                                const int sidx = ((lane & 1) << 2) | (lane & 2) | ((lane & 4) >> 2);
-                                mypart[tt + sidx] = P;
-                            }
+                            const u64 P = warp_reduce_tile(S, mytr, lane);
+                            if (lane < kTT) mypart[tt + lane] = P;
                         }
                     }
                 }
                 if (p.snr) {
-                    __syncthreads();
                     if (active) {
+                        group_barrier(ww);
                         // warps of one template share its ns samples; fixed summation order over warps
                         const u64* pb = part64 + (size_t)buf * W * kTS;
                         for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
@@ -211,7 +267,7 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
                     *reinterpret_cast<u64*>(yo + 2 * s) = Y[f];
                 }
             }
-            if (p.snr) __syncthreads();   // part buffers are reused by the next round
+            if (p.snr && active) group_barrier(ww);   // part rows are rewritten in the next round
         }
     }
 }

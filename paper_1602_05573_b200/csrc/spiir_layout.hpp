@@ -31,6 +31,7 @@ struct WarpWork {        // what one warp does in one round of one CTA item
 struct HostLayout {
     int F = 0;                          // register slots (filters) per thread
     int W = 0;                          // warps of one CTA = warp tiles processed side by side
+    int NC = 1;                         // shifted window copies = floats per shared-memory load
     int64_t n_tiles = 0;                // warp tiles
     int64_t n_slots = 0;                // n_tiles * F * 32
     std::vector<float> ar;              // [n_slots] Re a1
@@ -42,74 +43,89 @@ struct HostLayout {
     // work list: items (one CTA at a time), each with >= 1 rounds of W warp entries
     std::vector<int32_t> item_round0;   // [n_items+1] first round of each item
     std::vector<WarpWork> work;         // [n_rounds * W]
-    double avg_conflict_degree = 0.0;   // mean over groups of max residue multiplicity (diagnostic)
+    double avg_conflict_degree = 0.0;   // mean over load phases of the max key multiplicity (diagnostic)
 };
 
-// Deal the delay-sorted filters `order` (indices into d) of one template into G groups of <= 32.
-// Returns group-major list: out[g] = filter indices of group g.
-inline void deal_groups(const int32_t* d, const std::vector<int64_t>& order, int G,
-                        std::vector<std::vector<int64_t>>& out, double& degree_sum)
+// Deal the delay-sorted filters `order` (indices into d) of one template into G groups of <= 32 lanes.
+// A group is read with one shared-memory load instruction of NC floats per lane (NC = 1, 2, 4 =
+// LDS.32/.64/.128 from NC shifted copies of the window); the hardware serves it in NC phases of
+// P = 32/NC consecutive lanes, and a phase is conflict-free iff its lanes' aligned addresses fall into
+// distinct NC-word bank groups, i.e. iff key(d) = ceil(d / NC) mod P is distinct (calls that start at a
+// sample index that is a multiple of NC; other alignments stay correct and may conflict).
+// Returns group-major list: out[g] = filter indices of group g, lanes in phase order.
+inline int conflict_key(int32_t d, int NC, int P) { return (int)(((int64_t)d + NC - 1) / NC % P); }
+
+inline void deal_groups(const int32_t* d, const std::vector<int64_t>& order, int G, int NC,
+                        std::vector<std::vector<int64_t>>& out, double& degree_sum, int64_t& n_phases)
 {
-    out.assign(G, {});
-    std::vector<std::vector<int64_t>> bucket(kWarp);
-    for (int64_t k : order) bucket[d[k] & 31].push_back(k);
-    std::vector<size_t> head(kWarp, 0);
+    const int P = kWarp / NC;              // lanes per phase = number of bank groups
+    const int NP = G * NC;                 // phases to fill
+    std::vector<std::vector<int64_t>> ph(NP);
+    std::vector<std::vector<int64_t>> bucket(P);
+    for (int64_t k : order) bucket[conflict_key(d[k], NC, P)].push_back(k);
+    std::vector<size_t> head(P, 0);
     const int64_t K = (int64_t)order.size();
-    // phase 1: perfect groups (one filter of every residue), only full groups of 32
+    // phase 1: perfect phases (one filter of every key), only full phases of P
     size_t perfect = bucket[0].size();
-    for (int r = 1; r < kWarp; ++r) perfect = std::min(perfect, bucket[r].size());
-    perfect = std::min<size_t>(perfect, (size_t)(K / kWarp));
-    perfect = std::min<size_t>(perfect, (size_t)G);
+    for (int r = 1; r < P; ++r) perfect = std::min(perfect, bucket[r].size());
+    perfect = std::min<size_t>(perfect, (size_t)(K / P));
+    perfect = std::min<size_t>(perfect, (size_t)NP);
     for (size_t g = 0; g < perfect; ++g)
-        for (int r = 0; r < kWarp; ++r) out[g].push_back(bucket[r][head[r]++]);
-    // phase 2: spread the remainder evenly over the remaining groups: least multiplicity of the
-    // residue first, then emptiest group, then lowest index; fullest residues first
-    const int G2 = G - (int)perfect;
+        for (int r = 0; r < P; ++r) ph[g].push_back(bucket[r][head[r]++]);
+    // phase 2: spread the remainder evenly over the remaining phases: least multiplicity of the
+    // key first, then emptiest phase, then lowest index; fullest keys first
+    const int G2 = NP - (int)perfect;
     if (G2 > 0) {
-        std::vector<int> rorder(kWarp);
+        std::vector<int> rorder(P);
         std::iota(rorder.begin(), rorder.end(), 0);
         std::stable_sort(rorder.begin(), rorder.end(), [&](int a, int b) {
             return bucket[a].size() - head[a] > bucket[b].size() - head[b];
         });
         std::vector<int> fill(G2, 0);
-        std::vector<int> mult((size_t)G2 * kWarp, 0);
-        // capacity per group: groups before the last tile's padding must be full; give every group
-        // ceil/floor share so padding lands in the last groups
-        const int64_t rem = K - (int64_t)perfect * kWarp;
+        std::vector<int> mult((size_t)G2 * P, 0);
+        // capacity per phase: all but the last phases are full, so that padding lands at the end
+        const int64_t rem = K - (int64_t)perfect * P;
         std::vector<int> cap(G2, 0);
         {
             int64_t left = rem;
-            for (int g = 0; g < G2; ++g) { cap[g] = (int)std::min<int64_t>(kWarp, left); left -= cap[g]; }
+            for (int g = 0; g < G2; ++g) { cap[g] = (int)std::min<int64_t>(P, left); left -= cap[g]; }
         }
         for (int r : rorder) {
             while (head[r] < bucket[r].size()) {
                 int best = -1;
                 for (int g = 0; g < G2; ++g) {
                     if (fill[g] >= cap[g]) continue;
-                    if (best < 0 || mult[(size_t)g * kWarp + r] < mult[(size_t)best * kWarp + r] ||
-                        (mult[(size_t)g * kWarp + r] == mult[(size_t)best * kWarp + r] && fill[g] < fill[best]))
+                    if (best < 0 || mult[(size_t)g * P + r] < mult[(size_t)best * P + r] ||
+                        (mult[(size_t)g * P + r] == mult[(size_t)best * P + r] && fill[g] < fill[best]))
                         best = g;
                 }
-                out[perfect + best].push_back(bucket[r][head[r]++]);
+                ph[perfect + best].push_back(bucket[r][head[r]++]);
                 ++fill[best];
-                ++mult[(size_t)best * kWarp + r];
+                ++mult[(size_t)best * P + r];
             }
         }
     }
-    for (int g = 0; g < G; ++g) {
-        int cnt[kWarp] = {0};
+    // groups = NC consecutive phases; a short phase is followed only by empty ones
+    out.assign(G, {});
+    std::vector<int> cnt(P);
+    for (int q = 0; q < NP; ++q) {
+        if (ph[q].empty()) continue;
+        std::fill(cnt.begin(), cnt.end(), 0);
         int mx = 0;
-        for (int64_t k : out[g]) mx = std::max(mx, ++cnt[d[k] & 31]);
-        degree_sum += out[g].empty() ? 0 : mx;
+        for (int64_t k : ph[q]) mx = std::max(mx, ++cnt[conflict_key(d[k], NC, P)]);
+        degree_sum += mx;
+        ++n_phases;
+        out[q / NC].insert(out[q / NC].end(), ph[q].begin(), ph[q].end());
     }
 }
 
 inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, const float* b0,
-                               const int32_t* d, int F, int W)
+                               const int32_t* d, int F, int W, int NC = 1)
 {
     HostLayout L;
     L.F = F;
     L.W = W;
+    L.NC = NC;
     const int64_t K = off[T];
     L.tile_begin.resize((size_t)T + 1);
     int64_t tiles = 0;
@@ -128,7 +144,7 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
     L.slot_of_filter.assign((size_t)K, -1);
 
     double degree_sum = 0.0;
-    int64_t n_groups = 0;
+    int64_t n_phases = 0;
     std::vector<int64_t> order;
     std::vector<std::vector<int64_t>> groups;
     for (int32_t t = 0; t < T; ++t) {
@@ -138,10 +154,9 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
         std::stable_sort(order.begin(), order.end(), [&](int64_t x, int64_t y) { return d[x] < d[y]; });
         const int64_t nt = L.tile_begin[t + 1] - L.tile_begin[t];
         const int G = (int)(nt * F);
-        deal_groups(d, order, G, groups, degree_sum);
+        deal_groups(d, order, G, NC, groups, degree_sum, n_phases);
         for (int g = 0; g < G; ++g) {
             if (groups[g].empty()) continue;
-            ++n_groups;
             // lanes in delay order inside the group (any order is equally conflict-free)
             const int64_t slot0 = (L.tile_begin[t] * F + g) * kWarp;
             for (size_t l = 0; l < groups[g].size(); ++l) {
@@ -154,15 +169,17 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
                 L.dly[s] = d[k];
                 L.slot_of_filter[k] = s;
             }
-            for (size_t l = groups[g].size(); l < (size_t)kWarp; ++l)   // null filters: broadcast read
-                L.dly[slot0 + (int64_t)l] = d[groups[g][0]];
+            for (size_t l = groups[g].size(); l < (size_t)kWarp; ++l) {   // null filters: broadcast read
+                const size_t first = l / (size_t)(kWarp / NC) * (size_t)(kWarp / NC);   // first lane of the phase
+                L.dly[slot0 + (int64_t)l] = d[groups[g][first < groups[g].size() ? first : 0]];
+            }
         }
         // entirely empty groups of the last tile: point them at the template's smallest delay
         for (int g = 0; g < G; ++g)
             if (groups[g].empty())
                 for (int l = 0; l < kWarp; ++l) L.dly[(L.tile_begin[t] * F + g) * kWarp + l] = d[order[0]];
     }
-    L.avg_conflict_degree = n_groups ? degree_sum / (double)n_groups : 0.0;
+    L.avg_conflict_degree = n_phases ? degree_sum / (double)n_phases : 0.0;
 
     // Work list.  Templates with <= W tiles share an item round with their neighbours (greedy, in bank
     // order); a template with more tiles gets an item of its own with several accumulate rounds.
