@@ -111,6 +111,16 @@ int spiir_bank_set_state(spiir_bank *bank, const float *y_dev, const float *hist
 /* Free everything the bank owns (synchronises the device).  NULL is a no-op. */
 int spiir_bank_destroy(spiir_bank *bank);
 
+/* Host-only diagnostic (no CUDA call): lay the bank out exactly as spiir_bank_create would for the given
+ * register blocking (filters_per_thread F in {2,4,8,16}, warps_per_cta W, window_copies NC in {1,2,4}) and
+ * report it.  slot_of_filter (nullable, [K] int64, HOST) receives the device slot of every caller filter;
+ * stats (nullable, [8] double, HOST) receives {n_slots, n_warp_tiles, n_cta_items, n_rounds,
+ * avg_conflict_degree (mean over load phases of the largest number of lanes on one bank group; 1 = conflict
+ * free), padding_fraction = 1 - K/n_slots, 0, 0}.  Same argument checks as spiir_bank_create. */
+int spiir_layout_probe(int32_t n_templates, const int64_t *filter_offsets, const int32_t *delays,
+                       int32_t filters_per_thread, int32_t warps_per_cta, int32_t window_copies,
+                       int64_t *slot_of_filter, double *stats);
+
 /* Introspection. */
 const char *spiir_last_error(void);      /* thread-local message of the last failing call */
 int64_t spiir_kernel_launches(void);     /* kernels this library has launched in this process */

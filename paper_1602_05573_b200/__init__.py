@@ -9,5 +9,5 @@ from .binding import (SpiirError, SpiirOptions, SpiirBank, spiir_bank_create, sp
                       spiir_filter_host, spiir_bank_reset, spiir_bank_destroy, spiir_bank_num_templates,
                       spiir_bank_num_filters, spiir_bank_max_delay, spiir_bank_get_state,
                       spiir_bank_set_state, spiir_kernel_launches, spiir_last_error, spiir_version,
-                      spiir_bank_last_path, load_library, library_path,
+                      spiir_bank_last_path, spiir_layout_probe, shard_templates, load_library, library_path,
                       PATH_AUTO, PATH_THROUGHPUT, PATH_SCAN, PATH_STREAM)

@@ -15,7 +15,7 @@ PATH_AUTO, PATH_THROUGHPUT, PATH_SCAN, PATH_STREAM = 0, 1, 2, 3
 EXPORTS = ["spiir_bank_create", "spiir_filter", "spiir_filter_host", "spiir_bank_reset",
            "spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay",
            "spiir_bank_get_state", "spiir_bank_set_state", "spiir_bank_destroy", "spiir_last_error",
-           "spiir_kernel_launches", "spiir_bank_last_path", "spiir_version"]
+           "spiir_kernel_launches", "spiir_bank_last_path", "spiir_version", "spiir_layout_probe"]
 
 
 class SpiirError(RuntimeError):
@@ -75,6 +75,8 @@ def load_library():
     lib.spiir_bank_last_path.restype = i32
     lib.spiir_bank_last_path.argtypes = [vp]
     lib.spiir_version.restype = i32
+    lib.spiir_layout_probe.restype = ctypes.c_int
+    lib.spiir_layout_probe.argtypes = [i32, vp, vp, i32, i32, i32, vp, vp]
     _lib = lib
     return lib
 
@@ -192,6 +194,39 @@ def spiir_last_error() -> str:
 
 def spiir_version() -> int:
     return int(load_library().spiir_version())
+
+
+def spiir_layout_probe(filter_offsets, delays, filters_per_thread: int = 8, warps_per_cta: int = 16,
+                       window_copies: int = 1):
+    """Host-only: the device layout spiir_bank_create would build.  -> (slot_of_filter int64 [K], stats dict)."""
+    off = np.ascontiguousarray(filter_offsets, dtype=np.int64)
+    d = np.ascontiguousarray(delays, dtype=np.int32)
+    if off.ndim != 1 or off.size < 1 or d.shape != (int(off[-1]),):
+        raise ValueError("filter_offsets must be [T+1] and delays must have filter_offsets[-1] entries")
+    slots = np.empty(d.size, dtype=np.int64)
+    stats = np.zeros(8, dtype=np.float64)
+    _check(load_library().spiir_layout_probe(off.size - 1, _ptr(off), _ptr(d), filters_per_thread, warps_per_cta,
+                                             window_copies, _ptr(slots), _ptr(stats)))
+    names = ("n_slots", "n_warp_tiles", "n_cta_items", "n_rounds", "avg_conflict_degree", "padding_fraction")
+    return slots, dict(zip(names, stats.tolist()))
+
+
+def shard_templates(filter_offsets, world_size: int):
+    """Template indices of every rank for multi-GPU runs: templates are independent, so the
+    bank is split by template with no data-path collective.  Longest-processing-time-first bin packing on the
+    filter counts K_t; deterministic (ties: lower template index, lower rank).  -> list of sorted int64 arrays."""
+    off = np.asarray(filter_offsets, dtype=np.int64)
+    if world_size < 1 or off.ndim != 1 or off.size < 2:
+        raise ValueError("need world_size >= 1 and filter_offsets [T+1]")
+    kt = np.diff(off)
+    order = np.lexsort((np.arange(kt.size), -kt))          # K_t descending, then index
+    load = [0] * world_size
+    parts = [[] for _ in range(world_size)]
+    for t in order.tolist():
+        r = min(range(world_size), key=lambda i: (load[i], i))
+        parts[r].append(t)
+        load[r] += int(kt[t])
+    return [np.sort(np.asarray(p, dtype=np.int64)) for p in parts]
 
 
 class SpiirBank:

@@ -340,6 +340,39 @@ const char* spiir_last_error(void) { return g_err; }
 int64_t spiir_kernel_launches(void) { return g_launches.load(); }
 int32_t spiir_version(void) { return 100; }
 
+int spiir_layout_probe(int32_t T, const int64_t* off, const int32_t* delays, int32_t F, int32_t W, int32_t NC,
+                       int64_t* slot_of_filter, double* stats)
+{
+    if (!off || !delays) return fail(SPIIR_EINVAL, "null argument");
+    if (T <= 0) return fail(SPIIR_EINVAL, "n_templates must be >= 1");
+    if (off[0] != 0) return fail(SPIIR_EINVAL, "filter_offsets[0] must be 0");
+    for (int32_t t = 0; t < T; ++t)
+        if (off[t + 1] <= off[t]) return fail(SPIIR_EINVAL, "template %d has no filters (offsets must increase)", t);
+    if (!valid_blocking(F, W)) return fail(SPIIR_EINVAL, "unsupported blocking: filters_per_thread %d with warps_per_cta %d", F, W);
+    if (NC != 1 && NC != 2 && NC != 4) return fail(SPIIR_EINVAL, "window_copies must be 1, 2 or 4");
+    const int64_t K = off[T];
+    for (int64_t k = 0; k < K; ++k)
+        if (delays[k] < 0) return fail(SPIIR_EINVAL, "negative delay at filter %lld", (long long)k);
+    HostLayout L;
+    try {
+        std::vector<float> zeros((size_t)2 * K, 0.f);
+        L = build_layout(T, off, zeros.data(), zeros.data(), delays, F, W, NC);
+    } catch (const std::bad_alloc&) {
+        return fail(SPIIR_ENOMEM, "out of host memory building the bank layout");
+    }
+    if (slot_of_filter) memcpy(slot_of_filter, L.slot_of_filter.data(), (size_t)K * sizeof(int64_t));
+    if (stats) {
+        stats[0] = (double)L.n_slots;
+        stats[1] = (double)L.n_tiles;
+        stats[2] = (double)(L.item_round0.size() - 1);
+        stats[3] = (double)(L.work.size() / (size_t)W);
+        stats[4] = L.avg_conflict_degree;
+        stats[5] = L.n_slots ? 1.0 - (double)K / (double)L.n_slots : 0.0;
+        stats[6] = stats[7] = 0.0;
+    }
+    return SPIIR_OK;
+}
+
 int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const float* a1, const float* b0,
                       const int32_t* delays, int32_t device, const spiir_options* opt)
 {

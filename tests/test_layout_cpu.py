@@ -1,0 +1,97 @@
+"""Host logic of the bank layout, through the host-only C-ABI call
+spiir_layout_probe: every filter gets exactly one slot inside its own template's warp tiles, padding is
+what the tile size demands, lanes are dealt so that shared-memory loads avoid bank conflicts, and a
+template's layout does not depend on its position in the bank."""
+import numpy as np
+import pytest
+
+import spiir_inputs
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import __graft_entry__ as entry
+    entry.build()
+    import paper_1602_05573_b200 as p
+    return p
+
+
+def tiles_of(counts, F):
+    per = 32 * F
+    return [(-(-k // per)) for k in counts]
+
+
+@pytest.mark.parametrize("F,W", [(2, 32), (4, 16), (4, 32), (8, 8), (8, 16), (16, 8)])
+@pytest.mark.parametrize("NC", [1, 2, 4])
+def test_slots_are_a_partial_permutation_inside_each_template(pkg, F, W, NC):
+    counts = [1, 31, 32, 33, 64, 100, 255, 256, 257, 700, 5000, 3]
+    inp = spiir_inputs.make_random_bank(77, counts, 8, d_max=300)
+    slots, st = pkg.spiir_layout_probe(inp.offsets, inp.delays, F, W, NC)
+    nt = tiles_of(counts, F)
+    assert st["n_warp_tiles"] == sum(nt) and st["n_slots"] == sum(nt) * 32 * F
+    assert len(set(slots.tolist())) == slots.size                      # one slot per filter
+    first = np.concatenate([[0], np.cumsum(nt)]) * 32 * F
+    for t, k in enumerate(counts):
+        s = slots[inp.offsets[t]:inp.offsets[t + 1]]
+        assert s.min() >= first[t] and s.max() < first[t + 1]          # inside its own tiles
+    assert st["padding_fraction"] == pytest.approx(1 - sum(counts) / st["n_slots"])
+    assert 1.0 <= st["avg_conflict_degree"] <= 32 / NC
+
+
+@pytest.mark.parametrize("NC,bound", [(1, 1.55), (2, 1.35), (4, 1.22)])
+def test_dealing_keeps_uniform_random_delays_nearly_conflict_free(pkg, NC, bound):
+    # cfg3-like template sizes and delays; an undealt warp of 32 random delays has degree ~3.4 (NC = 1)
+    inp = spiir_inputs.make_config(3, n_templates=64, n_samples=8)
+    _, st = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, NC)
+    assert st["padding_fraction"] == 0.0
+    assert st["avg_conflict_degree"] < bound
+    # measure the phases directly from the slots: lanes of one load phase must mostly have distinct keys
+    slots, _ = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, NC)
+    d_of_slot = np.full(int(st["n_slots"]), -1, np.int64)
+    d_of_slot[slots] = inp.delays
+    P = 32 // NC
+    key = (-(-d_of_slot // NC)) % P
+    deg = [np.bincount(ph, minlength=P).max() for ph in key.reshape(-1, P)]
+    assert np.mean(deg) == pytest.approx(st["avg_conflict_degree"], rel=1e-12)
+
+
+def test_structured_delays_are_conflict_free(pkg):
+    inp = spiir_inputs.make_config(2, n_templates=8, n_samples=8)      # chirp bank: consecutive delays
+    for NC in (1, 2, 4):
+        _, st = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, NC)
+        assert st["avg_conflict_degree"] < 1.2
+
+
+def test_layout_of_a_template_is_independent_of_its_position(pkg):
+    inp = spiir_inputs.make_random_bank(5, [256, 100, 512, 33, 1024], 8, d_max=2000)
+    perm = np.array([3, 0, 4, 2, 1])
+    a, _ = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, 2)
+    pin = inp.select_templates(perm)
+    b, _ = pkg.spiir_layout_probe(pin.offsets, pin.delays, 8, 16, 2)
+    nt = tiles_of(np.diff(inp.offsets), 8)
+    base_a = np.concatenate([[0], np.cumsum(nt)]) * 256
+    base_b = np.concatenate([[0], np.cumsum(np.array(nt)[perm])]) * 256
+    for j, t in enumerate(perm):
+        rel_a = a[inp.offsets[t]:inp.offsets[t + 1]] - base_a[t]
+        rel_b = b[pin.offsets[j]:pin.offsets[j + 1]] - base_b[j]
+        assert np.array_equal(rel_a, rel_b)
+
+
+def test_work_list_counts(pkg):
+    # 4096 x 1024 filters, F = 8, W = 16: 4 warp tiles per template, 4 templates per CTA item
+    off = np.arange(0, 129) * 1024
+    d = (np.arange(128 * 1024) * 7919 % 16384).astype(np.int32)
+    _, st = pkg.spiir_layout_probe(off, d, 8, 16, 2)
+    assert st["n_warp_tiles"] == 512 and st["n_cta_items"] == 32 and st["n_rounds"] == 32
+    # a template larger than a CTA gets an item of its own with several rounds
+    _, st = pkg.spiir_layout_probe(np.array([0, 10000]), np.zeros(10000, np.int32), 8, 16, 1)
+    assert st["n_warp_tiles"] == 40 and st["n_cta_items"] == 1 and st["n_rounds"] == 3
+
+
+def test_probe_validates_arguments(pkg):
+    with pytest.raises(pkg.SpiirError):
+        pkg.spiir_layout_probe(np.array([0, 2]), np.array([0, -1], np.int32))
+    with pytest.raises(pkg.SpiirError):
+        pkg.spiir_layout_probe(np.array([0, 2]), np.zeros(2, np.int32), 3, 16, 1)
+    with pytest.raises(pkg.SpiirError):
+        pkg.spiir_layout_probe(np.array([0, 2]), np.zeros(2, np.int32), 8, 16, 3)
