@@ -27,7 +27,7 @@ def test_shard_templates_balances_and_partitions():
         loads = np.array([kt[p].sum() for p in parts])
         assert loads.max() - loads.min() <= kt.max()                       # LPT bound
         assert all(np.array_equal(p, np.sort(p)) for p in parts)
-    assert [p.tolist() for p in pkg.shard_templates(np.array([0, 5, 5 + 9, 5 + 9 + 9]), 2)] == [[1], [0, 2]]
+    assert [p.tolist() for p in pkg.shard_templates(np.array([0, 5, 5 + 9, 5 + 9 + 9]), 2)] == [[0, 1], [2]]
     with pytest.raises(ValueError):
         pkg.shard_templates(inp.offsets, 0)
 
