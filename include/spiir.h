@@ -116,7 +116,8 @@ int spiir_bank_destroy(spiir_bank *bank);
  * report it.  slot_of_filter (nullable, [K] int64, HOST) receives the device slot of every caller filter;
  * stats (nullable, [8] double, HOST) receives {n_slots, n_warp_tiles, n_cta_items, n_rounds,
  * avg_conflict_degree (mean over load phases of the largest number of lanes on one bank group; 1 = conflict
- * free), padding_fraction = 1 - K/n_slots, 0, 0}.  Same argument checks as spiir_bank_create. */
+ * free), padding_fraction = 1 - K/n_slots, uniform_groups (1 if every warp position always belongs to the
+ * same template shape, which enables per-template barriers), 0}.  Same argument checks as spiir_bank_create. */
 int spiir_layout_probe(int32_t n_templates, const int64_t *filter_offsets, const int32_t *delays,
                        int32_t filters_per_thread, int32_t warps_per_cta, int32_t window_copies,
                        int64_t *slot_of_filter, double *stats);

@@ -207,7 +207,8 @@ def spiir_layout_probe(filter_offsets, delays, filters_per_thread: int = 8, warp
     stats = np.zeros(8, dtype=np.float64)
     _check(load_library().spiir_layout_probe(off.size - 1, _ptr(off), _ptr(d), filters_per_thread, warps_per_cta,
                                              window_copies, _ptr(slots), _ptr(stats)))
-    names = ("n_slots", "n_warp_tiles", "n_cta_items", "n_rounds", "avg_conflict_degree", "padding_fraction")
+    names = ("n_slots", "n_warp_tiles", "n_cta_items", "n_rounds", "avg_conflict_degree", "padding_fraction",
+             "uniform_groups")
     return slots, dict(zip(names, stats.tolist()))
 
 

@@ -55,6 +55,7 @@ cudaError_t upload(T** dst, const std::vector<T>& v)
 struct spiir_bank {
     int device = 0;
     int F = 8, W = 16, NC = 1;
+    bool uniform_groups = true;
     bool gmem_only = false;          // the history alone exceeds shared memory: x is read through L1/L2
     bool configured[2] = {false, false};
     int64_t T = 0, K = 0, D = 0, n_slots = 0, n_tiles = 0;
@@ -217,6 +218,7 @@ FilterParams base_params(const spiir_bank* bk)
     FilterParams p{};
     p.ar = bk->ar; p.ai2 = bk->ai2; p.b = bk->b; p.dly = bk->dly;
     p.item_round0 = bk->item_round0; p.work = bk->work; p.n_items = bk->n_items;
+    p.uniform_groups = bk->uniform_groups ? 1 : 0;
     return p;
 }
 
@@ -368,7 +370,8 @@ int spiir_layout_probe(int32_t T, const int64_t* off, const int32_t* delays, int
         stats[3] = (double)(L.work.size() / (size_t)W);
         stats[4] = L.avg_conflict_degree;
         stats[5] = L.n_slots ? 1.0 - (double)K / (double)L.n_slots : 0.0;
-        stats[6] = stats[7] = 0.0;
+        stats[6] = L.uniform_groups ? 1.0 : 0.0;
+        stats[7] = 0.0;
     }
     return SPIIR_OK;
 }
@@ -458,6 +461,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->n_tiles = L.n_tiles;
     bk->n_items = (int32_t)(L.item_round0.size() - 1);
     bk->avg_conflict_degree = L.avg_conflict_degree;
+    bk->uniform_groups = L.uniform_groups;
     if (e == cudaSuccess) e = upload(&bk->ar, L.ar);
     if (e == cudaSuccess) e = upload(&bk->ai2, L.ai2);
     if (e == cudaSuccess) e = upload(&bk->b, L.b);

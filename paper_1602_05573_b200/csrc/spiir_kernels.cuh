@@ -45,6 +45,7 @@ struct FilterParams {
     const int32_t* item_round0;   // [n_items + 1]
     const WarpWork* work;         // [n_rounds * W]
     int32_t n_items;
+    int32_t uniform_groups;       // 1: per-template named barriers; 0: CTA-wide barriers (mixed group shapes)
     // state: per segment s (blockIdx.y) read y_in + s*y_in_stride, write y_out + s*y_out_stride
     const float* y_in;      // [2 n_slots] per segment; nullptr = zero state
     float* y_out;           // nullptr = do not store
@@ -245,8 +246,9 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
                     }
                 }
                 if (p.snr) {
+                    if (!p.uniform_groups) __syncthreads();
                     if (active) {
-                        group_barrier(ww);
+                        if (p.uniform_groups) group_barrier(ww);
                         // warps of one template share its ns samples; fixed summation order over warps
                         const u64* pb = part64 + (size_t)buf * W * kTS;
                         for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
@@ -267,7 +269,10 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
                     *reinterpret_cast<u64*>(yo + 2 * s) = Y[f];
                 }
             }
-            if (p.snr && active) group_barrier(ww);   // part rows are rewritten in the next round
+            if (p.snr) {                               // part rows are rewritten in the next round
+                if (!p.uniform_groups) __syncthreads();
+                else if (active) group_barrier(ww);
+            }
         }
     }
 }

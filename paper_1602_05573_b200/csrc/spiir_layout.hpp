@@ -43,6 +43,7 @@ struct HostLayout {
     // work list: items (one CTA at a time), each with >= 1 rounds of W warp entries
     std::vector<int32_t> item_round0;   // [n_items+1] first round of each item
     std::vector<WarpWork> work;         // [n_rounds * W]
+    bool uniform_groups = true;         // every warp position has the same (first, count) in all rounds it is active in
     double avg_conflict_degree = 0.0;   // mean over load phases of the max key multiplicity (diagnostic)
 };
 
@@ -211,6 +212,18 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
         }
     }
     flush();
+    // Named per-template barriers are only safe when a warp position always belongs to the same group shape:
+    // otherwise a fast warp could enter a hardware barrier that a slower group of another shape still uses.
+    {
+        std::vector<int32_t> first(W, -1), count(W, -1);
+        for (size_t i = 0; i < L.work.size(); ++i) {
+            const WarpWork& w = L.work[i];
+            if (w.tile < 0) continue;
+            const int pos = (int)(i % (size_t)W);
+            if (first[pos] < 0) { first[pos] = w.first; count[pos] = w.count; }
+            else if (first[pos] != w.first || count[pos] != w.count) { L.uniform_groups = false; break; }
+        }
+    }
     return L;
 }
 

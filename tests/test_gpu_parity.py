@@ -216,6 +216,18 @@ def test_cfg4_tiny_chunks(env, path):
     check(got, ref)
 
 
+def test_mixed_template_sizes_over_many_cta_items(env):
+    # more CTA items than SMs, every item a different mix of template sizes: CTAs walk through several items whose
+    # warp groups differ (regression: named barriers shared between groups of different shape)
+    inp = spiir_inputs.make_config(4, n_templates=2500, n_samples=96)
+    kt = np.diff(inp.offsets)
+    rows = np.sort(np.argsort(kt)[np.linspace(0, 2499, 20).astype(int)])
+    ref = env[1].run_inputs(inp.select_templates(rows))
+    for F in (0, 4):
+        got = run_gpu(env, inp, chunks=[16] * 6, path=1, F=F, rows=rows)
+        check(got, ref)
+
+
 # ------------------------------------------------------------------ oracle-free invariants
 def test_template_permutation_equivariance_and_determinism(env):
     inp = spiir_inputs.make_random_bank(21, [256, 100, 512, 33, 256, 1024, 64], 3000, d_max=2000)
