@@ -39,6 +39,18 @@ UNIT = "filter-samples/s"
 FLOPS_PER_FILTER_SAMPLE = 12          # complex*complex 6 + real*complex 2 + complex add 2 + sum 2
 N_SM, LANES, BOOST_HZ = 148, 128, 1.965e9   # B200: SMs x FP32 lanes x 2 flops x clocks.max.sm (MEASURED_PEAKS.json sm_max_mhz)
 FP32_PEAK_TFLOPS = N_SM * LANES * 2 * BOOST_HZ / 1e12    # 74.4 TFLOP/s, derivation in DESIGN.md section 7
+# dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch (cfg3, default blocking, 4096 samples)
+# from the committed ncu --set full capture profiles/r01b_filter_kernel_full.md: 135.1 MB + 115.5 MB
+NCU_TRAFFIC_CFG3_LAUNCH = 250.6e6
+
+
+def measured_hbm_peak():
+    """(GB/s, source): the driver-measured copy bandwidth of this pool's B200s, else the profiling guide's fallback."""
+    try:
+        d = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
 def workload_name(inp):
@@ -158,6 +170,8 @@ def run_ours(args):
         perm = rng.permutation(inp.n_templates)
         inp = inp.select_templates(perm)               # same distributions, different bank per rank
     N, L, T = inp.n_samples, inp.chunk, inp.n_templates
+    if args.path == 0 and L <= 64 and inp.n_filters >= (1 << 20):
+        args.path = pkg.PATH_STREAM            # tiny chunks over a large bank: the HBM-bound streaming blocking
     opt = pkg.SpiirOptions(path=args.path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta,
                            window_copies=args.window_copies)
     bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, local_rank, opt)
@@ -212,12 +226,35 @@ def run_ours(args):
     fs_call = inp.n_filters * L
     avg_call_s = float(np.mean(call_ms)) * 1e-3
     achieved_tflops = FLOPS_PER_FILTER_SAMPLE * fs_call / avg_call_s / 1e12
+    launches_per_call = max(1.0, launches / float(args.steps * n_calls))      # kernel launches of one spiir_filter call
+    traffic = args.ncu_traffic_bytes
+    default_blocking = not (args.filters_per_thread or args.warps_per_cta or args.window_copies or args.path)
+    if traffic is None and args.config == 3 and default_blocking:
+        traffic = NCU_TRAFFIC_CFG3_LAUNCH
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved_tflops / FP32_PEAK_TFLOPS, "traffic": args.ncu_traffic_bytes,
-                "kernel": "spiir_filter_kernel", "launch_ms": avg_call_s * 1e3,
+                "frac": achieved_tflops / FP32_PEAK_TFLOPS, "traffic": traffic,
+                "kernel": "spiir_filter_kernel", "launch_ms": avg_call_s * 1e3 / launches_per_call,
+                "launches_per_call": launches_per_call, "call_ms": avg_call_s * 1e3,
+                "algorithmic_flop_per_launch": FLOPS_PER_FILTER_SAMPLE * fs_call / launches_per_call,
+                "algorithmic_hbm_bytes_per_launch": (8.0 * T * L + 36.0 * inp.n_filters * launches_per_call) / launches_per_call,
+                "reachable_frac_register_file": 0.599,   # profiles/r01_fp32_pipe_probe.md: the 4-instruction body alone
                 "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1965 MHz (clocks.max.sm); no driver-measured FP32 peak exists",
                 "issue_slot_util": 8 * fs_call / avg_call_s / (N_SM * LANES * BOOST_HZ),
                 "hbm_write_gbs": 8.0 * T * L / avg_call_s / 1e9}
+
+    call_us = np.sort(np.asarray(call_ms)) * 1e3
+    latency = {"calls": int(call_us.size), "samples_per_call": int(L), "p50_us": float(np.percentile(call_us, 50)),
+               "p99_us": float(np.percentile(call_us, 99)), "max_us": float(call_us[-1]),
+               "real_time_us_per_call": 1e6 * L / spiir_inputs.FS}
+    if L <= 64:
+        # tiny chunks: every call streams the whole bank through the SMs once -> HBM roofline
+        bytes_call = inp.n_filters * 40.0 + 8.0 * T * L + 4.0 * L     # 24 B coefficients + 8 B state in + 8 B state out per filter
+        peak_gbs, peak_src = measured_hbm_peak()
+        roofline = {"bound": "hbm", "achieved": bytes_call / avg_call_s / 1e9, "peak": peak_gbs, "unit": "GB/s",
+                    "frac": bytes_call / avg_call_s / 1e9 / peak_gbs, "traffic": args.ncu_traffic_bytes,
+                    "kernel": "spiir_filter_kernel", "launch_ms": avg_call_s * 1e3 / launches_per_call,
+                    "launches_per_call": launches_per_call, "call_ms": avg_call_s * 1e3, "peak_source": peak_src,
+                    "algorithmic_bytes_per_call": bytes_call}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": elapsed_ms_max / args.steps, "higher_is_better": True,
@@ -227,7 +264,7 @@ def run_ours(args):
                              % (T * N * 8 / 1e9, inp.n_filters * 28 / 1e6),
                        "snr_buffer": "whole [T][N]" if keep_whole else "per-chunk [T][L] reused"},
             "pct_of_fp32_fma_peak": 100.0 * FLOPS_PER_FILTER_SAMPLE * value / world / (FP32_PEAK_TFLOPS * 1e12),
-            "gpu_launches": int(launches), "roofline": roofline, "clocks": clocks.summary()}
+            "gpu_launches": int(launches), "roofline": roofline, "latency": latency, "clocks": clocks.summary()}
 
     # ---- end to end through the public host-buffer entry (H2D + kernels + D2H inside the timed region)
     if not args.no_e2e:

@@ -54,7 +54,7 @@ typedef struct spiir_options {
     int32_t filters_per_thread; /* 0 = choose; else 2, 4, 8 or 16 (register blocking of the throughput kernel) */
     int32_t scan_segments;      /* 0 = choose; else time segments per call for SPIIR_PATH_SCAN */
     int32_t warps_per_cta;      /* 0 = choose; else 8, 16 or 32; valid (filters_per_thread, warps_per_cta) pairs:
-                                   (16,8) (8,8) (8,16) (4,16) (4,32) (2,32) */
+                                   (16,8) (8,8) (8,16) (4,8) (4,16) (4,32) (2,32) */
     int32_t window_copies;      /* 0 = choose; else 1, 2 or 4 shifted copies of the input window in shared memory
                                    (= floats per shared-memory load); falls back if they do not fit */
     int32_t reserved[2];        /* must be 0 */

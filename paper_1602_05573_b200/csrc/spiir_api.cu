@@ -146,19 +146,20 @@ int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
 // a 16 384-sample chunk behind a 16 383-sample history allows only one).
 const void* select_kernel(int F, int W, int NC, bool g)
 {
-#define SPIIR_VARIANT(F_, W_)                                                                  \
+#define SPIIR_VARIANT(F_, W_, M_)                                                              \
     if (F == F_ && W == W_) {                                                                  \
-        if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true>;                       \
-        if (NC == 4) return (const void*)spiir_filter_kernel<F_, W_, 4, false>;                \
-        if (NC == 2) return (const void*)spiir_filter_kernel<F_, W_, 2, false>;                \
-        return (const void*)spiir_filter_kernel<F_, W_, 1, false>;                             \
+        if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true, M_>;                   \
+        if (NC == 4) return (const void*)spiir_filter_kernel<F_, W_, 4, false, M_>;            \
+        if (NC == 2) return (const void*)spiir_filter_kernel<F_, W_, 2, false, M_>;            \
+        return (const void*)spiir_filter_kernel<F_, W_, 1, false, M_>;                         \
     }
-    SPIIR_VARIANT(16, 8)
-    SPIIR_VARIANT(8, 8)
-    SPIIR_VARIANT(8, 16)
-    SPIIR_VARIANT(4, 16)
-    SPIIR_VARIANT(4, 32)
-    SPIIR_VARIANT(2, 32)
+    SPIIR_VARIANT(16, 8, 1)
+    SPIIR_VARIANT(8, 8, 2)
+    SPIIR_VARIANT(8, 16, 1)
+    SPIIR_VARIANT(4, 8, 3)
+    SPIIR_VARIANT(4, 16, 1)
+    SPIIR_VARIANT(4, 32, 1)
+    SPIIR_VARIANT(2, 32, 1)
 #undef SPIIR_VARIANT
     return nullptr;
 }
@@ -421,8 +422,9 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->device = device;
     bk->opt = o;
     bk->T = T; bk->K = K; bk->D = D;
-    bk->F = choose_F(T, off, o.filters_per_thread);
-    bk->W = o.warps_per_cta ? o.warps_per_cta : default_warps(bk->F);
+    const bool stream = (o.path == SPIIR_PATH_STREAM);     // tiny chunks: small CTAs, several per SM
+    bk->F = stream && !o.filters_per_thread ? 4 : choose_F(T, off, o.filters_per_thread);
+    bk->W = o.warps_per_cta ? o.warps_per_cta : (stream ? 8 : default_warps(bk->F));
     if (!valid_blocking(bk->F, bk->W)) {
         const int F = bk->F, W = bk->W;
         free_bank(bk);
@@ -443,8 +445,11 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         const int64_t hist = round_up(D, 4) + 4 + 48;
         const int64_t kMinSub = 2048;
         bk->NC = 1;
-        for (int nc : {4, 2})
+        for (int nc : {4, 2}) {
+            if (stream) break;                              // one copy: room for more CTAs per SM
+
             if ((hist + kMinSub) * 4 * nc <= room) { bk->NC = nc; break; }
+        }
         if (o.window_copies == 1 || o.window_copies == 2 || o.window_copies == 4)
             if ((hist + kTS) * 4 * o.window_copies <= room) bk->NC = o.window_copies;
         bk->gmem_only = (hist + kTS) * 4 > room;

@@ -159,11 +159,15 @@ __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_l
 }
 
 // Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
-template <int F, int W, int NC, bool GMEM_X>
-__global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterParams p)
+// MINB = CTAs the register allocation must leave room for on one SM (tiny-chunk streaming: several small CTAs
+// per SM overlap one CTA's coefficient loads with another's arithmetic).
+template <int F, int W, int NC, bool GMEM_X, int MINB = 1>
+__global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const FilterParams p)
 {
     static_assert(!GMEM_X || NC == 1, "the global-memory window variant reads scalars");
     constexpr int kThreads = kWarp * W;
+    // named barriers make the CTA claim all 16 hardware barriers of the SM: only where one CTA owns the SM
+    constexpr bool kNamed = (MINB == 1);
     extern __shared__ __align__(16) float smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int seg = blockIdx.y;
@@ -246,9 +250,9 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
                     }
                 }
                 if (p.snr) {
-                    if (!p.uniform_groups) __syncthreads();
+                    if (!kNamed || !p.uniform_groups) __syncthreads();
                     if (active) {
-                        if (p.uniform_groups) group_barrier(ww);
+                        if (kNamed && p.uniform_groups) group_barrier(ww);
                         // warps of one template share its ns samples; fixed summation order over warps
                         const u64* pb = part64 + (size_t)buf * W * kTS;
                         for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
@@ -270,7 +274,7 @@ __global__ void __launch_bounds__(kWarp * W) spiir_filter_kernel(const FilterPar
                 }
             }
             if (p.snr) {                               // part rows are rewritten in the next round
-                if (!p.uniform_groups) __syncthreads();
+                if (!kNamed || !p.uniform_groups) __syncthreads();
                 else if (active) group_barrier(ww);
             }
         }
@@ -297,14 +301,28 @@ __global__ void spiir_scan_carry_kernel(const float* __restrict__ ar, const floa
     // c[0] is the carried state itself (segment 0 starts from it)
     c[2 * s] = (float)cr;
     c[2 * s + 1] = (float)ci;
-    for (int32_t q = 0; q + 1 < n_seg; ++q) {
-        const double zr = (double)z[(int64_t)q * 2 * n_slots + 2 * s], zi = (double)z[(int64_t)q * 2 * n_slots + 2 * s + 1];
-        const double nr = pr * cr - pi * ci + zr, ni = pr * ci + pi * cr + zi;
-        // continue from the float32-rounded carry: that is the state segment q+1 really starts from
-        cr = (double)(float)nr;
-        ci = (double)(float)ni;
-        c[(int64_t)(q + 1) * 2 * n_slots + 2 * s] = (float)nr;
-        c[(int64_t)(q + 1) * 2 * n_slots + 2 * s + 1] = (float)ni;
+    // the carries are a dependent chain, the loads of z are not: fetch them kB at a time ahead of the chain
+    constexpr int kB = 16;
+    for (int32_t q0 = 0; q0 + 1 < n_seg; q0 += kB) {
+        float zr[kB], zi[kB];
+#pragma unroll
+        for (int i = 0; i < kB; ++i) {
+            const int32_t q = min(q0 + i, n_seg - 2);
+            zr[i] = z[(int64_t)q * 2 * n_slots + 2 * s];
+            zi[i] = z[(int64_t)q * 2 * n_slots + 2 * s + 1];
+        }
+#pragma unroll
+        for (int i = 0; i < kB; ++i) {
+            const int32_t q = q0 + i;
+            if (q + 1 < n_seg) {
+                const double nr = pr * cr - pi * ci + (double)zr[i], ni = pr * ci + pi * cr + (double)zi[i];
+                // continue from the float32-rounded carry: that is the state segment q+1 really starts from
+                cr = (double)(float)nr;
+                ci = (double)(float)ni;
+                c[(int64_t)(q + 1) * 2 * n_slots + 2 * s] = (float)nr;
+                c[(int64_t)(q + 1) * 2 * n_slots + 2 * s + 1] = (float)ni;
+            }
+        }
     }
 }
 
