@@ -66,6 +66,7 @@ struct spiir_bank {
     float *ar = nullptr, *ai2 = nullptr, *b = nullptr, *y = nullptr;
     int32_t* dly = nullptr;
     int32_t* item_round0 = nullptr;
+    int32_t* canon = nullptr;
     WarpWork* work = nullptr;
     int64_t* slot_of_filter = nullptr;
     // input tape: tape[cur][0..pos) holds the most recent samples, the next chunk is appended at pos
@@ -99,7 +100,7 @@ void free_bank(spiir_bank* bk)
 {
     if (!bk) return;
     cudaFree(bk->ar); cudaFree(bk->ai2); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
-    cudaFree(bk->item_round0); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
+    cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
     cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
     cudaFree(bk->hx); cudaFree(bk->hsnr);
     if (bk->hstream) cudaStreamDestroy(bk->hstream);
@@ -220,6 +221,7 @@ FilterParams base_params(const spiir_bank* bk)
     p.ar = bk->ar; p.ai2 = bk->ai2; p.b = bk->b; p.dly = bk->dly;
     p.item_round0 = bk->item_round0; p.work = bk->work; p.n_items = bk->n_items;
     p.uniform_groups = bk->uniform_groups ? 1 : 0;
+    p.canon = bk->canon;
     return p;
 }
 
@@ -321,16 +323,16 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
 int choose_F(int32_t T, const int64_t* off, int requested)
 {
     if (requested == 2 || requested == 4 || requested == 8 || requested == 16) return requested;
-    // least padded work; F = 8 is the fastest inner loop, F = 4 pays ~4 % more reduction overhead
+    // Least padded work, weighted by the measured speed of the inner loops on a padding-free bank (cfg3:
+    // F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 / 32 warps 44 % of FP32 peak).
     double best = 0;
-    int bestF = 8;
-    for (int F : {8, 4}) {
+    int bestF = 0;
+    for (int F : {16, 8, 4}) {
         const int64_t per = 32LL * F;
         double padded = 0;
         for (int32_t t = 0; t < T; ++t) padded += (double)((off[t + 1] - off[t] + per - 1) / per * per);
-        padded *= (F == 8 ? 1.0 : 1.04);
-        if (bestF == 8 && F == 8) { best = padded; continue; }
-        if (padded < best) { best = padded; bestF = F; }
+        padded *= (F == 16 ? 1.0 : (F == 8 ? 1.05 : 1.22));
+        if (!bestF || padded < best) { best = padded; bestF = F; }
     }
     return bestF;
 }
@@ -473,6 +475,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     if (e == cudaSuccess) e = upload(&bk->dly, L.dly);
     if (e == cudaSuccess) e = upload(&bk->item_round0, L.item_round0);
     if (e == cudaSuccess) e = upload(&bk->work, L.work);
+    if (e == cudaSuccess) e = upload(&bk->canon, L.canon);
     if (e == cudaSuccess) e = upload(&bk->slot_of_filter, L.slot_of_filter);
     if (e == cudaSuccess) e = cudaMalloc((void**)&bk->y, (size_t)std::max<int64_t>(L.n_slots, 1) * 2 * sizeof(float));
     if (e == cudaSuccess) e = cudaMemset(bk->y, 0, (size_t)std::max<int64_t>(L.n_slots, 1) * 2 * sizeof(float));

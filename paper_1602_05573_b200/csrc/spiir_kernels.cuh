@@ -26,7 +26,10 @@ namespace spiir {
 typedef unsigned long long u64;
 
 constexpr int kTT = 8;        // samples per register tile
-constexpr int kTS = 64;       // samples per super tile (cross-warp combine + output granularity)
+constexpr int kTS = 64;       // granularity of launches and segments on the host side (multiple of every super tile)
+// samples per super tile (cross-warp combine + output granularity): W * super tile = 512 partial sums per buffer
+__host__ __device__ constexpr int super_tile(int W) { return W <= 8 ? 64 : 32; }
+constexpr int kPB = 3;        // partial-sum buffers per warp (3: a warp may run one super tile ahead of its template's slowest)
 
 __device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
 __device__ __forceinline__ u64 fmul2(u64 a, u64 b) { u64 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
@@ -45,7 +48,8 @@ struct FilterParams {
     const int32_t* item_round0;   // [n_items + 1]
     const WarpWork* work;         // [n_rounds * W]
     int32_t n_items;
-    int32_t uniform_groups;       // 1: per-template named barriers; 0: CTA-wide barriers (mixed group shapes)
+    int32_t uniform_groups;       // 1: per-template mbarriers, no CTA-wide barrier; 0: CTA-wide barriers (mixed group shapes)
+    const int32_t* canon;         // [2W] (first, count) of every warp position (uniform_groups only)
     // state: per segment s (blockIdx.y) read y_in + s*y_in_stride, write y_out + s*y_out_stride
     const float* y_in;      // [2 n_slots] per segment; nullptr = zero state
     float* y_out;           // nullptr = do not store
@@ -138,24 +142,51 @@ __device__ __forceinline__ u64 warp_reduce_tile(u64 (&S)[kTT], u64* __restrict__
     return P;
 }
 
-// Barrier over the warps of one template in the current round (they sit on different SM sub-partitions;
-// templates drift apart freely, so one template's reduction overlaps the others' arithmetic).  Groups of
-// >= 2 warps start at least 2 warps apart, so first/2 is a unique hardware barrier id in 0..15.
-__device__ __forceinline__ void group_barrier(const WarpWork& ww)
+// mbarrier helpers (shared::cta).  The warps of one template hand their partial sums to each other through
+// "full" barriers: lane 0 of every warp arrives after the warp has written a super tile, all lanes wait before
+// they read it.  Nobody ever waits for the slowest template of the CTA, only for the slowest warp of its own.
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(u64* bar, int count)
 {
-    if (ww.count > 1) asm volatile("bar.sync %0, %1;" ::"r"(ww.first >> 1), "r"(ww.count * kWarp) : "memory");
-    else __syncwarp();
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(u64* bar)
+{
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n .reg .pred p;\n"
+        "WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        " @p bra DONE_%=;\n bra WAIT_%=;\n"
+        "DONE_%=:\n}" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+
+// Sum the partial rows of the warps of one template for ns samples and store them (fixed order over warps).
+// The ns samples are shared out over the lanes of the template's warps.
+template <int TS>
+__device__ __forceinline__ void cross_warp_store(const u64* __restrict__ pb, const WarpWork& ww, int warp, int lane, int ns,
+                                                 u64* __restrict__ out, bool accumulate)
+{
+    for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
+        u64 acc = pb[(size_t)ww.first * TS + s];
+        for (int w = 1; w < ww.count; ++w) acc = fadd2(acc, pb[(size_t)(ww.first + w) * TS + s]);
+        if (accumulate) acc = fadd2(out[s], acc);
+        out[s] = acc;
+    }
 }
 
 // Shared memory of the filter kernel, in this order:
-//   NC window copies of `cstride` floats each (absent when GMEM_X), W transpose scratches, 2 x W x kTS partial sums
+//   NC window copies of `cstride` floats each (absent when GMEM_X), W transpose scratches, kPB x W x kTS partial sums,
+//   W x kPB mbarriers
 __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_len, bool gmem_x, int64_t* cstride_out)
 {
     // copy stride = 0 mod 32 floats: every copy starts on bank 0, as the lane dealing assumes
     const int64_t cstride = gmem_x ? 0 : ((win_len + 16 + 31) / 32 * 32);
     if (cstride_out) *cstride_out = cstride;
     return (size_t)(gmem_x ? 0 : NC * cstride) * sizeof(float) + (size_t)W * kTrWarp * sizeof(u64) +
-           2ull * W * kTS * sizeof(u64);
+           (size_t)kPB * W * super_tile(W) * sizeof(u64) + (size_t)W * kPB * sizeof(u64);
 }
 
 // Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
@@ -166,8 +197,8 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
 {
     static_assert(!GMEM_X || NC == 1, "the global-memory window variant reads scalars");
     constexpr int kThreads = kWarp * W;
-    // named barriers make the CTA claim all 16 hardware barriers of the SM: only where one CTA owns the SM
-    constexpr bool kNamed = (MINB == 1);
+    constexpr bool kAsync = (MINB == 1);
+    constexpr int TS = super_tile(W);
     extern __shared__ __align__(16) float smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int seg = blockIdx.y;
@@ -203,8 +234,17 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
         xs = smem;
     }
     u64* trbuf = reinterpret_cast<u64*>(smem + (GMEM_X ? 0 : NC * cstride));   // [W][kTrWarp]
-    u64* part64 = trbuf + (size_t)W * kTrWarp;                                 // [2][W][kTS]
+    u64* part64 = trbuf + (size_t)W * kTrWarp;                                 // [kPB][W][TS]
+    u64* bars = part64 + (size_t)kPB * W * TS;                                // [W][kPB], indexed by a group's first warp
     u64* mytr = trbuf + (size_t)warp * kTrWarp;
+    // per-template hand-over without any CTA-wide barrier: only where one CTA owns the SM and all rounds have one shape
+    const bool async = kAsync && p.uniform_groups && p.snr;
+    if (async && tid < W) {
+        const int first = p.canon[2 * tid], count = p.canon[2 * tid + 1];
+        if (first == tid && count > 0)
+            for (int b = 0; b < kPB; ++b) mbar_init(bars + tid * kPB + b, count);
+    }
+    unsigned use = 0;                                                          // super tiles this warp has produced
     __syncthreads();
 
     const bool last_seg = (t0 + nseg >= p.n);
@@ -232,36 +272,62 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                 }
             }
             const bool accumulate = (r > r0);
-            int buf = 0;
-            for (int64_t st = 0; st < nseg; st += kTS, buf ^= 1) {
-                const int ns = (int)min((int64_t)kTS, nseg - st);
+            u64* const out_row = reinterpret_cast<u64*>(p.snr) + (int64_t)ww.row * p.ld + t0;
+            if (async) {
                 if (active) {
-                    u64* mypart = part64 + ((size_t)buf * W + warp) * kTS;
+                    int prev_ns = 0;
+                    int64_t prev_st = 0;
+                    unsigned prev_use = 0;
+                    u64* mybars = bars + ww.first * kPB;
+                    for (int64_t st = 0; st < nseg; st += TS) {
+                        const int ns = (int)min((int64_t)TS, nseg - st);
+                        const unsigned i = use++;
+                        u64* mypart = part64 + ((size_t)(i % kPB) * W + warp) * TS;
 #pragma unroll 1
-                    for (int tt = 0; tt < ns; tt += kTT) {
-                        u64 S[kTT];
-                        const int nv = ns - tt;
-                        if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
-                        else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
-                        if (p.snr) {
+                        for (int tt = 0; tt < ns; tt += kTT) {
+                            u64 S[kTT];
+                            const int nv = ns - tt;
+                            if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
+                            else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
                             const u64 P = warp_reduce_tile(S, mytr, lane);
                             if (lane < kTT) mypart[tt + lane] = P;
                         }
+                        // finish the previous super tile before announcing this one (keeps 3 buffers sufficient)
+                        if (prev_ns) {
+                            mbar_wait(mybars + prev_use % kPB, (prev_use / kPB) & 1);
+                            cross_warp_store<TS>(part64 + (size_t)(prev_use % kPB) * W * TS, ww, warp, lane, prev_ns, out_row + prev_st, accumulate);
+                        }
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(mybars + i % kPB);
+                        prev_ns = ns; prev_st = st; prev_use = i;
+                    }
+                    if (prev_ns) {
+                        mbar_wait(mybars + prev_use % kPB, (prev_use / kPB) & 1);
+                        cross_warp_store<TS>(part64 + (size_t)(prev_use % kPB) * W * TS, ww, warp, lane, prev_ns, out_row + prev_st, accumulate);
                     }
                 }
-                if (p.snr) {
-                    if (!kNamed || !p.uniform_groups) __syncthreads();
+            } else {
+                int buf = 0;
+                for (int64_t st = 0; st < nseg; st += TS, buf ^= 1) {
+                    const int ns = (int)min((int64_t)TS, nseg - st);
                     if (active) {
-                        if (kNamed && p.uniform_groups) group_barrier(ww);
-                        // warps of one template share its ns samples; fixed summation order over warps
-                        const u64* pb = part64 + (size_t)buf * W * kTS;
-                        for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
-                            u64 acc = pb[(size_t)ww.first * kTS + s];
-                            for (int w = 1; w < ww.count; ++w) acc = fadd2(acc, pb[(size_t)(ww.first + w) * kTS + s]);
-                            u64* out = reinterpret_cast<u64*>(p.snr) + (int64_t)ww.row * p.ld + t0 + st + s;
-                            if (accumulate) acc = fadd2(*out, acc);
-                            *out = acc;
+                        u64* mypart = part64 + ((size_t)buf * W + warp) * TS;
+#pragma unroll 1
+                        for (int tt = 0; tt < ns; tt += kTT) {
+                            u64 S[kTT];
+                            const int nv = ns - tt;
+                            if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
+                            else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
+                            if (p.snr) {
+                                const u64 P = warp_reduce_tile(S, mytr, lane);
+                                if (lane < kTT) mypart[tt + lane] = P;
+                            }
                         }
+                    }
+                    if (p.snr) {
+                        __syncthreads();
+                        if (active)
+                            cross_warp_store<TS>(part64 + (size_t)buf * W * TS, ww, warp, lane, ns, out_row + st, accumulate);
                     }
                 }
             }
@@ -273,10 +339,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                     *reinterpret_cast<u64*>(yo + 2 * s) = Y[f];
                 }
             }
-            if (p.snr) {                               // part rows are rewritten in the next round
-                if (!kNamed || !p.uniform_groups) __syncthreads();
-                else if (active) group_barrier(ww);
-            }
+            if (p.snr && !async) __syncthreads();      // part rows are rewritten in the next round
         }
     }
 }

@@ -43,6 +43,7 @@ struct HostLayout {
     // work list: items (one CTA at a time), each with >= 1 rounds of W warp entries
     std::vector<int32_t> item_round0;   // [n_items+1] first round of each item
     std::vector<WarpWork> work;         // [n_rounds * W]
+    std::vector<int32_t> canon;         // [2W] (first, count) of every warp position when uniform_groups, else (-1, 0)
     bool uniform_groups = true;         // every warp position has the same (first, count) in all rounds it is active in
     double avg_conflict_degree = 0.0;   // mean over load phases of the max key multiplicity (diagnostic)
 };
@@ -222,6 +223,11 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
             const int pos = (int)(i % (size_t)W);
             if (first[pos] < 0) { first[pos] = w.first; count[pos] = w.count; }
             else if (first[pos] != w.first || count[pos] != w.count) { L.uniform_groups = false; break; }
+        }
+        L.canon.assign((size_t)2 * W, 0);
+        for (int w = 0; w < W; ++w) {
+            L.canon[2 * w] = L.uniform_groups ? first[w] : -1;
+            L.canon[2 * w + 1] = L.uniform_groups && first[w] >= 0 ? count[w] : 0;
         }
     }
     return L;
