@@ -170,7 +170,9 @@ bool valid_blocking(int F, int W) { return select_kernel(F, W, 1, false) != null
 int default_warps(int F) { return F >= 16 ? 8 : (F == 8 ? 16 : 32); }
 
 // shared memory besides the window copies
-size_t fixed_smem(int W) { return filter_smem_bytes(W, 1, 0, true, nullptr); }
+// variants compiled for several CTAs per SM keep the CTA-wide barrier and need only 2 partial-sum buffers
+int part_buffers(int F, int W) { return (W == 8 && (F == 8 || F == 4)) ? 2 : kPB; }
+size_t fixed_smem(int F, int W) { return filter_smem_bytes(W, 1, 0, true, nullptr, part_buffers(F, W)); }
 
 // allow the kernel to use all opt-in shared memory (once per variant and bank)
 int configure_kernel(spiir_bank* bk, bool g, const void** fn)
@@ -230,12 +232,14 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
 {
     const size_t smem_cap = bk->smem_optin;
     // window floats per copy that fit beside the reduction buffers (a copy is padded by up to 47 floats)
-    const int64_t max_win = ((int64_t)smem_cap - (int64_t)fixed_smem(bk->W)) / (4 * bk->NC) - 48;
+    const int64_t max_win = ((int64_t)smem_cap - (int64_t)fixed_smem(bk->F, bk->W)) / (4 * bk->NC) - 48;
     const bool gmem = bk->gmem_only;          // history alone does not fit: read x through L1/L2
     int path = bk->opt.path;
-    // ---- how much time-parallelism is needed to fill the machine?
+    // ---- how much time-parallelism is needed to fill the machine?  The scan path does the recurrence twice, so it
+    // only pays when the bank leaves at least half of the SMs idle (cfg2: 128 items on 148 SMs run 1.7x faster
+    // sequentially).
     int64_t n_seg = 1;
-    if (path == SPIIR_PATH_SCAN || (path == SPIIR_PATH_AUTO && bk->n_items < bk->n_sm && n >= 4 * kTS)) {
+    if (path == SPIIR_PATH_SCAN || (path == SPIIR_PATH_AUTO && 2 * bk->n_items <= bk->n_sm && n >= 4 * kTS)) {
         const int64_t max_seg = std::max<int64_t>(1, n / kTS);
         int64_t want = bk->opt.scan_segments > 0 ? bk->opt.scan_segments
                                                  : ((int64_t)2 * bk->n_sm + bk->n_items - 1) / bk->n_items;
@@ -257,7 +261,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
             p.y_in = bk->y; p.y_out = bk->y; p.y_in_stride = 0; p.y_out_stride = 0; p.store_last_only = 1;
             p.xwin = xwin + off; p.w0 = w0; p.n = ns; p.seg_len = ns;
             p.snr = snr + 2 * off; p.ld = ld;
-            const size_t smem = filter_smem_bytes(bk->W, bk->NC, w0 + ns, gmem, nullptr);
+            const size_t smem = filter_smem_bytes(bk->W, bk->NC, w0 + ns, gmem, nullptr, part_buffers(bk->F, bk->W));
             int occ = 1;
             int rc = cached_occupancy(bk, gmem, smem, &occ);
             if (rc) return rc;
@@ -282,7 +286,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
         CU_TRY(cudaMalloc((void**)&bk->cbuf, bytes));
         bk->scan_cap_seg = n_seg;
     }
-    const size_t smem = filter_smem_bytes(bk->W, bk->NC, w0 + seg_len, gmem, nullptr);
+    const size_t smem = filter_smem_bytes(bk->W, bk->NC, w0 + seg_len, gmem, nullptr, part_buffers(bk->F, bk->W));
     int occ = 1;
     int rc = cached_occupancy(bk, gmem, smem, &occ);
     if (rc) return rc;
@@ -443,7 +447,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     // Window copies: as many (4, 2, 1 = LDS.128/.64/.32 per filter) as leave room for >= kMinSub samples per
     // launch behind the history; none at all (global-memory reads) if not even one copy of the history fits.
     {
-        const int64_t room = (int64_t)bk->smem_optin - (int64_t)fixed_smem(bk->W);
+        const int64_t room = (int64_t)bk->smem_optin - (int64_t)fixed_smem(bk->F, bk->W);
         const int64_t hist = round_up(D, 4) + 4 + 48;
         const int64_t kMinSub = 2048;
         bk->NC = 1;

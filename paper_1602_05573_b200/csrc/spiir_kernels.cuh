@@ -180,13 +180,14 @@ __device__ __forceinline__ void cross_warp_store(const u64* __restrict__ pb, con
 // Shared memory of the filter kernel, in this order:
 //   NC window copies of `cstride` floats each (absent when GMEM_X), W transpose scratches, kPB x W x kTS partial sums,
 //   W x kPB mbarriers
-__host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_len, bool gmem_x, int64_t* cstride_out)
+__host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_len, bool gmem_x, int64_t* cstride_out,
+                                                     int part_buffers = kPB)
 {
     // copy stride = 0 mod 32 floats: every copy starts on bank 0, as the lane dealing assumes
     const int64_t cstride = gmem_x ? 0 : ((win_len + 16 + 31) / 32 * 32);
     if (cstride_out) *cstride_out = cstride;
     return (size_t)(gmem_x ? 0 : NC * cstride) * sizeof(float) + (size_t)W * kTrWarp * sizeof(u64) +
-           (size_t)kPB * W * super_tile(W) * sizeof(u64) + (size_t)W * kPB * sizeof(u64);
+           (size_t)part_buffers * W * super_tile(W) * sizeof(u64) + (size_t)W * kPB * sizeof(u64);
 }
 
 // Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
@@ -235,7 +236,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     }
     u64* trbuf = reinterpret_cast<u64*>(smem + (GMEM_X ? 0 : NC * cstride));   // [W][kTrWarp]
     u64* part64 = trbuf + (size_t)W * kTrWarp;                                 // [kPB][W][TS]
-    u64* bars = part64 + (size_t)kPB * W * TS;                                // [W][kPB], indexed by a group's first warp
+    u64* bars = part64 + (size_t)(kAsync ? kPB : 2) * W * TS;                                // [W][kPB], indexed by a group's first warp
     u64* mytr = trbuf + (size_t)warp * kTrWarp;
     // per-template hand-over without any CTA-wide barrier: only where one CTA owns the SM and all rounds have one shape
     const bool async = kAsync && p.uniform_groups && p.snr;
