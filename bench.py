@@ -6,7 +6,7 @@
 One "step" = one pass of the whole hot path over one batch of synthetic input: the streaming run of
 BASELINE.json:configs[3] (4096 templates x 1024 filters, 262 144 float32 samples fed as 16 chunks of 16 384
 with state carry), i.e. 16 spiir_filter calls = 1.0995e12 filter-samples.  Inputs are resident in HBM when the
-timed region starts (`value`); `e2e` repeats the measurement through spiir_filter_host with host buffers
+timed region starts (`value`); `e2e` repeats the measurement through spiir_filter_host_async / spiir_bank_host_sync with host buffers
 (H2D of every chunk and D2H of every SNR block inside the timed region).  Prints ONE JSON line.
 
 N > 1 (torchrun, one rank per GPU): templates are independent, so every rank filters
@@ -269,14 +269,17 @@ def run_ours(args):
     # ---- end to end through the public host-buffer entry (H2D + kernels + D2H inside the timed region)
     if not args.no_e2e:
         xh = torch.from_numpy(inp.x).pin_memory()
-        outh = torch.empty((T, L), dtype=torch.complex64).pin_memory()
+        outh = torch.empty((2, T, L), dtype=torch.complex64).pin_memory()      # results land here, two chunks deep
         xh_np, outh_np = xh.numpy(), outh.numpy()
 
         def e2e_step():
             bank.reset()
-            for c0 in range(0, N, L):
+            for i, c0 in enumerate(range(0, N, L)):
                 n = min(L, N - c0)
-                pkg.spiir_filter_host(bank.handle, xh_np[c0:c0 + n], outh_np[:, :n])
+                # enqueue H2D of the chunk, the kernels and the D2H of SNR[:, chunk]; the copies of chunk i overlap
+                # the kernels of chunk i+1
+                pkg.spiir_filter_host_async(bank.handle, xh_np[c0:c0 + n], outh_np[i & 1, :, :n])
+            pkg.spiir_bank_host_sync(bank.handle)                               # every result of the step is in host memory
 
         e2e_step()
         barrier()
@@ -291,7 +294,7 @@ def run_ours(args):
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         line["e2e"] = {"value": world * fs_step * e2e_steps / float(tt.item()), "unit": UNIT,
                        "h2d_bytes_per_step": int(N * 4), "d2h_bytes_per_step": int(T * N * 8),
-                       "steps": e2e_steps, "api": "spiir_filter_host (pinned host buffers)"}
+                       "steps": e2e_steps, "api": "spiir_filter_host_async per chunk + spiir_bank_host_sync per step (pinned host buffers)"}
 
     # ---- the CPU oracle beside it (rank 0, N = 1 only): a reported baseline, not the target
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -95,6 +95,13 @@ int spiir_filter(spiir_bank *bank, const float *x_dev, int64_t n, float *snr_dev
  * Buffers may be pageable or pinned.  Returns after the results are in snr_host. */
 int spiir_filter_host(spiir_bank *bank, const float *x_host, int64_t n, float *snr_host, int64_t ld);
 
+/* The same, but returns as soon as the work is enqueued on the bank's own streams: the copies of this chunk's
+ * results overlap the kernels of the next chunk ("overlapping technology").  x_host and snr_host
+ * must be PINNED host memory and stay untouched until spiir_bank_host_sync returns; calls may be issued back to
+ * back (they are ordered).  spiir_bank_host_sync blocks until every enqueued chunk's results are in host memory. */
+int spiir_filter_host_async(spiir_bank *bank, const float *x_host, int64_t n, float *snr_host, int64_t ld);
+int spiir_bank_host_sync(spiir_bank *bank);
+
 /* Zero the filter state and the input history (a cold bank again); enqueued on the stream. */
 int spiir_bank_reset(spiir_bank *bank, void *stream);
 

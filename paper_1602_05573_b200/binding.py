@@ -15,7 +15,8 @@ PATH_AUTO, PATH_THROUGHPUT, PATH_SCAN, PATH_STREAM = 0, 1, 2, 3
 EXPORTS = ["spiir_bank_create", "spiir_filter", "spiir_filter_host", "spiir_bank_reset",
            "spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay",
            "spiir_bank_get_state", "spiir_bank_set_state", "spiir_bank_destroy", "spiir_last_error",
-           "spiir_kernel_launches", "spiir_bank_last_path", "spiir_version", "spiir_layout_probe"]
+           "spiir_kernel_launches", "spiir_bank_last_path", "spiir_version", "spiir_layout_probe",
+           "spiir_filter_host_async", "spiir_bank_host_sync"]
 
 
 class SpiirError(RuntimeError):
@@ -59,6 +60,10 @@ def load_library():
     lib.spiir_filter.argtypes = [vp, vp, i64, vp, i64, vp]
     lib.spiir_filter_host.restype = ctypes.c_int
     lib.spiir_filter_host.argtypes = [vp, vp, i64, vp, i64]
+    lib.spiir_filter_host_async.restype = ctypes.c_int
+    lib.spiir_filter_host_async.argtypes = [vp, vp, i64, vp, i64]
+    lib.spiir_bank_host_sync.restype = ctypes.c_int
+    lib.spiir_bank_host_sync.argtypes = [vp]
     lib.spiir_bank_reset.restype = ctypes.c_int
     lib.spiir_bank_reset.argtypes = [vp, vp]
     for name in ("spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay"):
@@ -132,8 +137,9 @@ def spiir_filter(bank, x, snr, ld: int | None = None, stream=None, n: int | None
                                        int(ld), _stream_handle(stream)))
 
 
-def spiir_filter_host(bank, x: np.ndarray, snr: np.ndarray | None = None) -> np.ndarray:
-    """Host-buffer entry: x float32 [n] numpy -> complex64 [T, n] numpy (H2D, kernels, D2H inside)."""
+def spiir_filter_host(bank, x: np.ndarray, snr: np.ndarray | None = None, asynchronous: bool = False) -> np.ndarray:
+    """Host-buffer entry: x float32 [n] numpy -> complex64 [T, n] numpy (H2D, kernels, D2H inside).
+    ``asynchronous`` = spiir_filter_host_async: x and snr must be pinned and stay untouched until spiir_bank_host_sync."""
     lib = load_library()
     x = np.ascontiguousarray(x, dtype=np.float32)
     T = int(lib.spiir_bank_num_templates(bank))
@@ -143,8 +149,16 @@ def spiir_filter_host(bank, x: np.ndarray, snr: np.ndarray | None = None) -> np.
             (snr.shape[1] > 1 and snr.strides[1] != 8):
         raise ValueError("snr must be complex64 [T, >=n] with unit column stride")
     ld = snr.strides[0] // 8 if T > 1 else max(snr.shape[1], x.size)
-    _check(lib.spiir_filter_host(bank, _ptr(x), x.size, _ptr(snr), ld))
+    _check((lib.spiir_filter_host_async if asynchronous else lib.spiir_filter_host)(bank, _ptr(x), x.size, _ptr(snr), ld))
     return snr
+
+
+def spiir_filter_host_async(bank, x: np.ndarray, snr: np.ndarray) -> np.ndarray:
+    return spiir_filter_host(bank, x, snr, asynchronous=True)
+
+
+def spiir_bank_host_sync(bank):
+    _check(load_library().spiir_bank_host_sync(bank))
 
 
 def spiir_bank_reset(bank, stream=None):

@@ -77,9 +77,13 @@ struct spiir_bank {
     float *zbuf = nullptr, *cbuf = nullptr;
     int64_t scan_cap_seg = 0;
     // host-path scratch
-    float *hx = nullptr, *hsnr = nullptr;
+    float* hx = nullptr;
+    float* hsnr[2] = {nullptr, nullptr};
     int64_t hx_cap = 0, hsnr_cap = 0;
-    cudaStream_t hstream = nullptr;
+    cudaStream_t hstream = nullptr, cstream = nullptr;
+    cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_reset = nullptr;
+    bool free_pending[2] = {false, false};
+    int64_t host_piece = 0;          // pieces enqueued so far by the host-buffer entry (ping-pong index)
     // device facts
     int n_sm = 0;
     size_t smem_optin = 0;
@@ -102,8 +106,14 @@ void free_bank(spiir_bank* bk)
     cudaFree(bk->ar); cudaFree(bk->ai2); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
     cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
     cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
-    cudaFree(bk->hx); cudaFree(bk->hsnr);
+    cudaFree(bk->hx); cudaFree(bk->hsnr[0]); cudaFree(bk->hsnr[1]);
+    for (int i = 0; i < 2; ++i) {
+        if (bk->ev_done[i]) cudaEventDestroy(bk->ev_done[i]);
+        if (bk->ev_free[i]) cudaEventDestroy(bk->ev_free[i]);
+    }
+    if (bk->ev_reset) cudaEventDestroy(bk->ev_reset);
     if (bk->hstream) cudaStreamDestroy(bk->hstream);
+    if (bk->cstream) cudaStreamDestroy(bk->cstream);
     delete bk;
 }
 
@@ -519,32 +529,78 @@ int spiir_filter(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, 
     return SPIIR_OK;
 }
 
-int spiir_filter_host(spiir_bank* bk, const float* x_host, int64_t n, float* snr_host, int64_t ld)
+int spiir_filter_host_async(spiir_bank* bk, const float* x_host, int64_t n, float* snr_host, int64_t ld)
 {
     if (!bk) return fail(SPIIR_EINVAL, "null bank");
     if (n < 0 || ld < n) return fail(SPIIR_EINVAL, "need 0 <= n <= ld");
     if (n == 0) return SPIIR_OK;
     if (!x_host || !snr_host) return fail(SPIIR_EINVAL, "null host pointer");
     CU_TRY(cudaSetDevice(bk->device));
-    if (!bk->hstream) CU_TRY(cudaStreamCreateWithFlags(&bk->hstream, cudaStreamNonBlocking));
+    if (!bk->hstream) {
+        CU_TRY(cudaStreamCreateWithFlags(&bk->hstream, cudaStreamNonBlocking));
+        CU_TRY(cudaStreamCreateWithFlags(&bk->cstream, cudaStreamNonBlocking));
+        CU_TRY(cudaEventCreateWithFlags(&bk->ev_reset, cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) {
+            CU_TRY(cudaEventCreateWithFlags(&bk->ev_done[i], cudaEventDisableTiming));
+            CU_TRY(cudaEventCreateWithFlags(&bk->ev_free[i], cudaEventDisableTiming));
+        }
+    }
+    // The chunk is filtered in pieces; the device-to-host copy of one piece (copy stream) overlaps the kernels of
+    // the next ("overlapping technology").  Two device buffers ping-pong.
+    int64_t piece = n;
+    if (n >= 4 * 2048) piece = round_up((n + 3) / 4, kTS);
     if (bk->hx_cap < n) {
+        CU_TRY(cudaStreamSynchronize(bk->hstream));
         cudaFree(bk->hx); bk->hx = nullptr; bk->hx_cap = 0;
         CU_TRY(cudaMalloc((void**)&bk->hx, (size_t)n * sizeof(float)));
         bk->hx_cap = n;
     }
-    const int64_t need = bk->T * n * 2;
+    const int64_t need = bk->T * piece * 2;
     if (bk->hsnr_cap < need) {
-        cudaFree(bk->hsnr); bk->hsnr = nullptr; bk->hsnr_cap = 0;
-        CU_TRY(cudaMalloc((void**)&bk->hsnr, (size_t)need * sizeof(float)));
+        CU_TRY(cudaStreamSynchronize(bk->hstream));
+        CU_TRY(cudaStreamSynchronize(bk->cstream));
+        for (int i = 0; i < 2; ++i) {
+            cudaFree(bk->hsnr[i]); bk->hsnr[i] = nullptr;
+        }
+        bk->hsnr_cap = 0;
+        for (int i = 0; i < 2; ++i) CU_TRY(cudaMalloc((void**)&bk->hsnr[i], (size_t)need * sizeof(float)));
         bk->hsnr_cap = need;
     }
     CU_TRY(cudaMemcpyAsync(bk->hx, x_host, (size_t)n * sizeof(float), cudaMemcpyHostToDevice, bk->hstream));
-    int rc = spiir_filter(bk, bk->hx, n, bk->hsnr, n, bk->hstream);
-    if (rc) return rc;
-    CU_TRY(cudaMemcpy2DAsync(snr_host, (size_t)ld * 8, bk->hsnr, (size_t)n * 8, (size_t)n * 8, (size_t)bk->T,
-                             cudaMemcpyDeviceToHost, bk->hstream));
-    CU_TRY(cudaStreamSynchronize(bk->hstream));
+    int j = 0;
+    for (int64_t off = 0; off < n; off += piece, ++j) {
+        const int64_t len = std::min(piece, n - off);
+        const int b = (int)((bk->host_piece + j) & 1);
+        if (bk->free_pending[b]) CU_TRY(cudaStreamWaitEvent(bk->hstream, bk->ev_free[b], 0));   // the last copy out of this buffer is done
+        int rc = spiir_filter(bk, bk->hx + off, len, bk->hsnr[b], len, bk->hstream);
+        if (rc) return rc;
+        CU_TRY(cudaEventRecord(bk->ev_done[b], bk->hstream));
+        CU_TRY(cudaStreamWaitEvent(bk->cstream, bk->ev_done[b], 0));
+        CU_TRY(cudaMemcpy2DAsync(snr_host + 2 * off, (size_t)ld * 8, bk->hsnr[b], (size_t)len * 8, (size_t)len * 8,
+                                 (size_t)bk->T, cudaMemcpyDeviceToHost, bk->cstream));
+        CU_TRY(cudaEventRecord(bk->ev_free[b], bk->cstream));
+        bk->free_pending[b] = true;
+    }
+    bk->host_piece += j;
     return SPIIR_OK;
+}
+
+int spiir_bank_host_sync(spiir_bank* bk)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    if (!bk->hstream) return SPIIR_OK;
+    CU_TRY(cudaSetDevice(bk->device));
+    CU_TRY(cudaStreamSynchronize(bk->hstream));
+    CU_TRY(cudaStreamSynchronize(bk->cstream));
+    bk->free_pending[0] = bk->free_pending[1] = false;
+    return SPIIR_OK;
+}
+
+int spiir_filter_host(spiir_bank* bk, const float* x_host, int64_t n, float* snr_host, int64_t ld)
+{
+    int rc = spiir_filter_host_async(bk, x_host, n, snr_host, ld);
+    if (rc) return rc;
+    return n > 0 ? spiir_bank_host_sync(bk) : SPIIR_OK;
 }
 
 int spiir_bank_reset(spiir_bank* bk, void* stream)
@@ -555,6 +611,10 @@ int spiir_bank_reset(spiir_bank* bk, void* stream)
     CU_TRY(cudaMemsetAsync(bk->y, 0, (size_t)std::max<int64_t>(bk->n_slots, 1) * 2 * sizeof(float), st));
     bk->pos = round_up(bk->D, 4);
     CU_TRY(cudaMemsetAsync(bk->tape[bk->cur], 0, (size_t)(bk->pos + 8) * sizeof(float), st));
+    if (bk->hstream) {      // the host-buffer entry works on the bank's own stream: order it behind this reset
+        CU_TRY(cudaEventRecord(bk->ev_reset, st));
+        CU_TRY(cudaStreamWaitEvent(bk->hstream, bk->ev_reset, 0));
+    }
     bk->poisoned = false;
     return SPIIR_OK;
 }

@@ -259,6 +259,24 @@ def test_checkpoint_resume(env):
     assert np.array_equal(snr.cpu().numpy().view(np.float32), full.view(np.float32))
 
 
+def test_async_host_entry_back_to_back(env):
+    pkg, oracle, torch = env
+    inp = spiir_inputs.make_random_bank(43, [128, 512, 70], 3 * 8192 + 100, d_max=900)
+    ref = oracle.run_inputs(inp)
+    xh = torch.from_numpy(inp.x).pin_memory()
+    out = torch.empty((3, inp.n_samples), dtype=torch.complex64).pin_memory()
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays) as bank:
+        pos = 0
+        for c in (8192, 8192, 100, 8192):                      # pieces inside a chunk, chunks back to back, no sync between
+            pkg.spiir_filter_host_async(bank.handle, xh.numpy()[pos:pos + c], out.numpy()[:, pos:pos + c])
+            pos += c
+        pkg.spiir_bank_host_sync(bank.handle)
+        check(out.numpy(), ref)
+        bank.reset()
+        again = pkg.spiir_filter_host(bank.handle, inp.x)      # synchronous entry, pageable memory
+        check(again, ref)                                      # another chunking: equal within tolerance, not bitwise
+
+
 def test_reset_and_host_entry(env):
     pkg, oracle, torch = env
     inp = spiir_inputs.make_random_bank(41, [128, 512], 5000, d_max=900)
