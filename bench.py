@@ -39,9 +39,9 @@ UNIT = "filter-samples/s"
 FLOPS_PER_FILTER_SAMPLE = 12          # complex*complex 6 + real*complex 2 + complex add 2 + sum 2
 N_SM, LANES, BOOST_HZ = 148, 128, 1.965e9   # B200: SMs x FP32 lanes x 2 flops x clocks.max.sm (MEASURED_PEAKS.json sm_max_mhz)
 FP32_PEAK_TFLOPS = N_SM * LANES * 2 * BOOST_HZ / 1e12    # 74.4 TFLOP/s, derivation in DESIGN.md section 7
-# dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch (cfg3, default blocking, 4096 samples)
-# from the committed ncu --set full capture profiles/r01b_filter_kernel_full.md: 135.1 MB + 115.5 MB
-NCU_TRAFFIC_CFG3_LAUNCH = 250.6e6
+# dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch (cfg3, default blocking, 8192 samples)
+# from the committed ncu --set full capture profiles/r01c_filter_kernel_full.md: 135.8 MB + 245.7 MB
+NCU_TRAFFIC_CFG3_LAUNCH = 381.6e6
 
 
 def measured_hbm_peak():
