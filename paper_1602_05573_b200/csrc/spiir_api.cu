@@ -67,6 +67,9 @@ struct spiir_bank {
     int32_t* dly = nullptr;
     int32_t* item_round0 = nullptr;
     int32_t* canon = nullptr;
+    int64_t* tile_begin = nullptr;   // [T+1] first warp tile of every template (streaming combine)
+    u64* stream_scratch = nullptr;   // [n_tiles][kStreamMax] per-tile partial sums (streaming path)
+    bool stream_configured = false;
     WarpWork* work = nullptr;
     int64_t* slot_of_filter = nullptr;
     // input tape: tape[cur][0..pos) holds the most recent samples, the next chunk is appended at pos
@@ -104,7 +107,7 @@ void free_bank(spiir_bank* bk)
 {
     if (!bk) return;
     cudaFree(bk->ar); cudaFree(bk->ai2); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
-    cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
+    cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->tile_begin); cudaFree(bk->stream_scratch); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
     cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
     cudaFree(bk->hx); cudaFree(bk->hsnr[0]); cudaFree(bk->hsnr[1]);
     for (int i = 0; i < 2; ++i) {
@@ -237,6 +240,43 @@ FilterParams base_params(const spiir_bank* bk)
     return p;
 }
 
+// Tiny chunk through the streaming kernels: independent warps + a combine pass.
+const void* select_stream_kernel(int F, int NC)
+{
+    if (F == 4) return NC == 2 ? (const void*)spiir_stream_kernel<4, 2, 3> : (const void*)spiir_stream_kernel<4, 1, 3>;
+    if (F == 8) return NC == 2 ? (const void*)spiir_stream_kernel<8, 2, 2> : (const void*)spiir_stream_kernel<8, 1, 2>;
+    return nullptr;
+}
+
+int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st)
+{
+    const void* fn = select_stream_kernel(bk->F, bk->NC);
+    if (!fn) return fail(SPIIR_EINVAL, "no streaming kernel for F=%d NC=%d", bk->F, bk->NC);
+    if (!bk->stream_configured) {
+        CU_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bk->smem_optin));
+        bk->stream_configured = true;
+    }
+    if (!bk->stream_scratch)
+        CU_TRY(cudaMalloc((void**)&bk->stream_scratch, (size_t)std::max<int64_t>(bk->n_tiles, 1) * kStreamMax * sizeof(u64)));
+    const size_t smem = stream_smem_bytes(bk->NC, w0 + n, nullptr);
+    int occ = 0;
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kWarp * kStreamWarps, smem));
+    if (occ < 1) return fail(SPIIR_ECUDA, "streaming kernel does not fit on an SM (smem %zu)", smem);
+    StreamParams p{};
+    p.ar = bk->ar; p.ai2 = bk->ai2; p.b = bk->b; p.dly = bk->dly; p.y = bk->y;
+    p.xwin = xwin; p.w0 = w0; p.n = (int32_t)n; p.n_tiles = bk->n_tiles; p.scratch = bk->stream_scratch;
+    const int64_t ctas = std::min<int64_t>((bk->n_tiles + kStreamWarps - 1) / kStreamWarps, (int64_t)bk->n_sm * occ);
+    void* args[] = {(void*)&p};
+    CU_TRY(cudaLaunchKernel(fn, dim3((unsigned)ctas, 1, 1), dim3(kWarp * kStreamWarps, 1, 1), args, smem, st));
+    const int64_t total = bk->T * n;
+    spiir_stream_combine_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(bk->stream_scratch, bk->tile_begin,
+                                                                             (int32_t)bk->T, (int32_t)n, snr, ld);
+    g_launches.fetch_add(2, std::memory_order_relaxed);
+    CU_TRY(cudaGetLastError());
+    bk->last_path = SPIIR_PATH_STREAM;
+    return SPIIR_OK;
+}
+
 // Run the filter kernels over n samples whose window starts at xwin (aligned), sample 0 at xwin[w0].
 int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st)
 {
@@ -245,6 +285,9 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     const int64_t max_win = ((int64_t)smem_cap - (int64_t)fixed_smem(bk->F, bk->W)) / (4 * bk->NC) - 48;
     const bool gmem = bk->gmem_only;          // history alone does not fit: read x through L1/L2
     int path = bk->opt.path;
+    if (path == SPIIR_PATH_STREAM && n <= kStreamMax && !gmem && select_stream_kernel(bk->F, bk->NC) &&
+        stream_smem_bytes(bk->NC, w0 + n, nullptr) <= smem_cap)
+        return run_stream(bk, xwin, w0, n, snr, ld, st);
     // ---- how much time-parallelism is needed to fill the machine?  The scan path does the recurrence twice, so it
     // only pays when the bank leaves at least half of the SMs idle (cfg2: 128 items on 148 SMs run 1.7x faster
     // sequentially).
@@ -490,6 +533,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     if (e == cudaSuccess) e = upload(&bk->item_round0, L.item_round0);
     if (e == cudaSuccess) e = upload(&bk->work, L.work);
     if (e == cudaSuccess) e = upload(&bk->canon, L.canon);
+    if (e == cudaSuccess) e = upload(&bk->tile_begin, L.tile_begin);
     if (e == cudaSuccess) e = upload(&bk->slot_of_filter, L.slot_of_filter);
     if (e == cudaSuccess) e = cudaMalloc((void**)&bk->y, (size_t)std::max<int64_t>(L.n_slots, 1) * 2 * sizeof(float));
     if (e == cudaSuccess) e = cudaMemset(bk->y, 0, (size_t)std::max<int64_t>(L.n_slots, 1) * 2 * sizeof(float));

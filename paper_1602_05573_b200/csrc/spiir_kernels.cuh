@@ -345,6 +345,106 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     }
 }
 
+// ---- tiny-chunk streaming (SPIIR_PATH_STREAM, n <= kStreamMax samples per call).
+// Every call streams the whole bank through the SMs once, so the path is bound by HBM and by per-round
+// overhead, not by arithmetic.  Warps are independent: a warp takes warp tiles round-robin, loads their
+// coefficients and state, advances the n samples, reduces over its 32 lanes and writes the tile's partial sums
+// to a scratch row; no barrier, no shared partial buffers.  spiir_stream_combine_kernel then adds the tiles of
+// every template in tile order (fixed order -> bitwise reproducible).
+constexpr int kStreamMax = 64;          // samples per call served by the streaming kernels
+constexpr int kStreamWarps = 8;         // warps per CTA
+
+struct StreamParams {
+    const float* ar; const float* ai2; const float* b; const int32_t* dly;
+    float* y;                     // state, updated in place
+    const float* xwin; int32_t w0; int32_t n;
+    int64_t n_tiles;
+    u64* scratch;                 // [n_tiles][kStreamMax] partial sums of every warp tile
+};
+
+__host__ __device__ inline size_t stream_smem_bytes(int NC, int64_t win_len, int64_t* cstride_out)
+{
+    const int64_t cstride = (win_len + 16 + 31) / 32 * 32;
+    if (cstride_out) *cstride_out = cstride;
+    return (size_t)(NC * cstride) * sizeof(float) + (size_t)kStreamWarps * kTrWarp * sizeof(u64);
+}
+
+template <int F, int NC, int MINB>
+__global__ void __launch_bounds__(kWarp * kStreamWarps, MINB) spiir_stream_kernel(const StreamParams p)
+{
+    constexpr int kThreads = kWarp * kStreamWarps;
+    extern __shared__ __align__(16) float smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int win_len = p.w0 + p.n;
+    int64_t cstride;
+    stream_smem_bytes(NC, win_len, &cstride);
+    {
+        const float4* src = reinterpret_cast<const float4*>(p.xwin);
+        const int n4 = (int)(cstride / 4), v4 = (win_len + 3) / 4;
+        for (int i = tid; i < n4; i += kThreads) {
+            const float4 v = i < v4 ? src[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+            reinterpret_cast<float4*>(smem)[i] = v;
+            if (NC > 1) {
+                const float e[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int c = 1; c < NC; ++c) {
+                    float* dst = smem + (int64_t)c * cstride + 4 * i - c;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (4 * i + q - c >= 0) dst[q] = e[q];
+                }
+            }
+        }
+    }
+    const float* xs = smem;
+    u64* mytr = reinterpret_cast<u64*>(smem + NC * cstride) + (size_t)warp * kTrWarp;
+    __syncthreads();
+
+    const int64_t n_warps = (int64_t)gridDim.x * kStreamWarps;
+    for (int64_t tile = (int64_t)blockIdx.x * kStreamWarps + warp; tile < p.n_tiles; tile += n_warps) {
+        float ar[F];
+        u64 AI[F], B[F], Y[F];
+        int xo[F];
+        const int64_t s0 = tile * F * kWarp + lane;
+#pragma unroll
+        for (int f = 0; f < F; ++f) {
+            const int64_t s = s0 + f * kWarp;
+            ar[f] = p.ar[s];
+            AI[f] = ld_pair(p.ai2 + 2 * s);
+            B[f] = ld_pair(p.b + 2 * s);
+            Y[f] = ld_pair(p.y + 2 * s);
+            const int p0 = p.w0 - p.dly[s];
+            const int c = p0 & (NC - 1);
+            xo[f] = (int)(c * cstride) + p0 - c;
+        }
+        u64* row = p.scratch + tile * kStreamMax;
+#pragma unroll 1
+        for (int tt = 0; tt < p.n; tt += kTT) {
+            u64 S[kTT];
+            const int nv = p.n - tt;
+            if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, tt, kTT);
+            else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, tt, nv);
+            const u64 P = warp_reduce_tile(S, mytr, lane);
+            if (lane < kTT) row[tt + lane] = P;
+        }
+#pragma unroll
+        for (int f = 0; f < F; ++f) *reinterpret_cast<u64*>(p.y + 2 * (s0 + f * kWarp)) = Y[f];
+    }
+}
+
+// SNR[t][j] = sum over the warp tiles of template t, in tile order, of scratch[tile][j].  One thread per (t, j).
+__global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, const int64_t* __restrict__ tile_begin,
+                                            int32_t n_templates, int32_t n, float* __restrict__ snr, int64_t ld)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (int64_t)n_templates * n) return;
+    const int32_t t = (int32_t)(i / n), j = (int32_t)(i % n);
+    const int64_t t0 = tile_begin[t], t1 = tile_begin[t + 1];
+    u64 acc = scratch[t0 * kStreamMax + j];
+    for (int64_t tile = t0 + 1; tile < t1; ++tile) acc = fadd2(acc, scratch[tile * kStreamMax + j]);
+    reinterpret_cast<u64*>(snr)[(int64_t)t * ld + j] = acc;
+}
+
 // ---- time-parallel scan: carry combine.  For every slot, given the carried state c_0 = y and the
 // zero-state end values z_p of segments p = 0..P-2 (all of length seg_len), produce the true start
 // states c_{p+1} = a1^seg_len * c_p + z_p.  Powers and the combine are evaluated in double from the

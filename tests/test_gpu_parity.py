@@ -72,7 +72,7 @@ def check(got, ref, tol=TOL):
 
 
 # ------------------------------------------------------------------ exact golden vector, all paths
-@pytest.mark.parametrize("path,F", [(1, 0), (1, 2), (1, 16), (2, 0)])
+@pytest.mark.parametrize("path,F", [(1, 0), (1, 2), (1, 16), (2, 0), (3, 0), (3, 8)])
 def test_p7_golden_vector_bitwise(env, path, F):
     rows, filters, x = [], [], None
     for line in (Path(__file__).parent / "golden" / "p7_dyadic.txt").read_text().splitlines():
@@ -205,7 +205,7 @@ def test_cfg3_full_size_subset_and_invariants(env):
 
 
 # ------------------------------------------------------------------ config 4: variable filter counts, 16-sample chunks
-@pytest.mark.parametrize("path", [0, 2])
+@pytest.mark.parametrize("path", [0, 2, 3])
 def test_cfg4_tiny_chunks(env, path):
     inp = spiir_inputs.make_config(4, n_templates=512, n_samples=1024)
     kt = np.diff(inp.offsets)
@@ -226,9 +226,26 @@ def test_mixed_template_sizes_over_many_cta_items(env):
     for F in (0, 4):
         got = run_gpu(env, inp, chunks=[16] * 6, path=1, F=F, rows=rows)
         check(got, ref)
+    # the streaming kernels (independent warps + combine) with ragged tiny chunks, and larger chunks in between
+    # that fall back to the blocked kernel on the same bank
+    got = run_gpu(env, inp, chunks=[16, 1, 7, 40, 0, 24, 8], path=3, rows=rows)
+    check(got, ref)
+    got = run_gpu(env, inp, chunks=[64, 32], path=3, F=8, rows=rows)
+    check(got, ref)
 
 
 # ------------------------------------------------------------------ oracle-free invariants
+def test_streaming_path_determinism_and_position_independence(env):
+    inp = spiir_inputs.make_random_bank(22, [256, 100, 512, 33, 256, 1024, 64, 2000], 160, d_max=2000)
+    a = run_gpu(env, inp, chunks=[16] * 10, path=3)
+    b = run_gpu(env, inp, chunks=[16] * 10, path=3)
+    assert np.array_equal(a.view(np.float32), b.view(np.float32))
+    perm = np.array([3, 6, 0, 7, 5, 1, 4, 2])
+    c = run_gpu(env, inp.select_templates(perm), chunks=[16] * 10, path=3)
+    assert np.array_equal(c.view(np.float32), a[perm].view(np.float32))
+    check(a, env[1].run_inputs(inp))
+
+
 def test_template_permutation_equivariance_and_determinism(env):
     inp = spiir_inputs.make_random_bank(21, [256, 100, 512, 33, 256, 1024, 64], 3000, d_max=2000)
     a = run_gpu(env, inp, chunks=[1000, 2000], path=1)
