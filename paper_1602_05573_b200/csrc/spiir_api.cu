@@ -243,8 +243,15 @@ FilterParams base_params(const spiir_bank* bk)
 // Tiny chunk through the streaming kernels: independent warps + a combine pass.
 const void* select_stream_kernel(int F, int NC)
 {
-    if (F == 4) return NC == 2 ? (const void*)spiir_stream_kernel<4, 2, 3> : (const void*)spiir_stream_kernel<4, 1, 3>;
-    if (F == 8) return NC == 2 ? (const void*)spiir_stream_kernel<8, 2, 2> : (const void*)spiir_stream_kernel<8, 1, 2>;
+#define SPIIR_STREAM(F_)                                                            \
+    if (F == F_) {                                                                  \
+        if (NC == 4) return (const void*)spiir_stream_kernel<F_, 4>;                \
+        if (NC == 2) return (const void*)spiir_stream_kernel<F_, 2>;                \
+        return (const void*)spiir_stream_kernel<F_, 1>;                             \
+    }
+    SPIIR_STREAM(4)
+    SPIIR_STREAM(8)
+#undef SPIIR_STREAM
     return nullptr;
 }
 
@@ -258,7 +265,8 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
     }
     if (!bk->stream_scratch)
         CU_TRY(cudaMalloc((void**)&bk->stream_scratch, (size_t)std::max<int64_t>(bk->n_tiles, 1) * kStreamMax * sizeof(u64)));
-    const size_t smem = stream_smem_bytes(bk->NC, w0 + n, nullptr);
+    const int kStreamWarps = stream_warps(bk->F);
+    const size_t smem = stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr);
     int occ = 0;
     CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kWarp * kStreamWarps, smem));
     if (occ < 1) return fail(SPIIR_ECUDA, "streaming kernel does not fit on an SM (smem %zu)", smem);
@@ -286,7 +294,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     const bool gmem = bk->gmem_only;          // history alone does not fit: read x through L1/L2
     int path = bk->opt.path;
     if (path == SPIIR_PATH_STREAM && n <= kStreamMax && !gmem && select_stream_kernel(bk->F, bk->NC) &&
-        stream_smem_bytes(bk->NC, w0 + n, nullptr) <= smem_cap)
+        stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr) <= smem_cap)
         return run_stream(bk, xwin, w0, n, snr, ld, st);
     // ---- how much time-parallelism is needed to fill the machine?  The scan path does the recurrence twice, so it
     // only pays when the bank leaves at least half of the SMs idle (cfg2: 128 items on 148 SMs run 1.7x faster
@@ -505,7 +513,11 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         const int64_t kMinSub = 2048;
         bk->NC = 1;
         for (int nc : {4, 2}) {
-            if (stream) break;                              // one copy: room for more CTAs per SM
+            if (stream) {                                   // sized for the streaming kernels (one big CTA per SM)
+                if (stream_smem_bytes(bk->F, nc, hist + kStreamMax, nullptr) <= bk->smem_optin &&
+                    (hist + 2048) * 4 * nc <= room) { bk->NC = nc; break; }
+                continue;
+            }
 
             if ((hist + kMinSub) * 4 * nc <= room) { bk->NC = nc; break; }
         }

@@ -352,7 +352,9 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
 // to a scratch row; no barrier, no shared partial buffers.  spiir_stream_combine_kernel then adds the tiles of
 // every template in tile order (fixed order -> bitwise reproducible).
 constexpr int kStreamMax = 64;          // samples per call served by the streaming kernels
-constexpr int kStreamWarps = 8;         // warps per CTA
+// warps per CTA (one CTA per SM; the warps never synchronise, a big CTA only shares the staged window): what the
+// register file allows
+__host__ __device__ constexpr int stream_warps(int F) { return F <= 4 ? 24 : 16; }
 
 struct StreamParams {
     const float* ar; const float* ai2; const float* b; const int32_t* dly;
@@ -362,22 +364,23 @@ struct StreamParams {
     u64* scratch;                 // [n_tiles][kStreamMax] partial sums of every warp tile
 };
 
-__host__ __device__ inline size_t stream_smem_bytes(int NC, int64_t win_len, int64_t* cstride_out)
+__host__ __device__ inline size_t stream_smem_bytes(int F, int NC, int64_t win_len, int64_t* cstride_out)
 {
     const int64_t cstride = (win_len + 16 + 31) / 32 * 32;
     if (cstride_out) *cstride_out = cstride;
-    return (size_t)(NC * cstride) * sizeof(float) + (size_t)kStreamWarps * kTrWarp * sizeof(u64);
+    return (size_t)(NC * cstride) * sizeof(float) + (size_t)stream_warps(F) * kTrWarp * sizeof(u64);
 }
 
-template <int F, int NC, int MINB>
-__global__ void __launch_bounds__(kWarp * kStreamWarps, MINB) spiir_stream_kernel(const StreamParams p)
+template <int F, int NC>
+__global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kernel(const StreamParams p)
 {
+    constexpr int kStreamWarps = stream_warps(F);
     constexpr int kThreads = kWarp * kStreamWarps;
     extern __shared__ __align__(16) float smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int win_len = p.w0 + p.n;
     int64_t cstride;
-    stream_smem_bytes(NC, win_len, &cstride);
+    stream_smem_bytes(F, NC, win_len, &cstride);
     {
         const float4* src = reinterpret_cast<const float4*>(p.xwin);
         const int n4 = (int)(cstride / 4), v4 = (win_len + 3) / 4;
@@ -417,6 +420,22 @@ __global__ void __launch_bounds__(kWarp * kStreamWarps, MINB) spiir_stream_kerne
             const int c = p0 & (NC - 1);
             xo[f] = (int)(c * cstride) + p0 - c;
         }
+        // Ask for the next tile of this warp now (its 8F cache lines, one or two per lane), so that its loads hit L1
+        // after this tile's arithmetic instead of waiting for HBM: the warps never have nothing in flight.
+        if (tile + n_warps < p.n_tiles) {
+            const int64_t t0n = (tile + n_warps) * F * kWarp;          // first slot of the next tile
+#pragma unroll
+            for (int q = 0; q < (8 * F + kWarp - 1) / kWarp; ++q) {
+                const int idx = lane + q * kWarp;
+                const float* line;
+                if (idx < F) line = p.ar + t0n + idx * kWarp;
+                else if (idx < 3 * F) line = p.ai2 + 2 * t0n + (idx - F) * kWarp;
+                else if (idx < 5 * F) line = p.b + 2 * t0n + (idx - 3 * F) * kWarp;
+                else if (idx < 6 * F) line = reinterpret_cast<const float*>(p.dly) + t0n + (idx - 5 * F) * kWarp;
+                else line = p.y + 2 * t0n + (idx - 6 * F) * kWarp;
+                if (idx < 8 * F) asm volatile("prefetch.global.L1 [%0];" ::"l"(line));
+            }
+        }
         u64* row = p.scratch + tile * kStreamMax;
 #pragma unroll 1
         for (int tt = 0; tt < p.n; tt += kTT) {
@@ -441,7 +460,15 @@ __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, con
     const int32_t t = (int32_t)(i / n), j = (int32_t)(i % n);
     const int64_t t0 = tile_begin[t], t1 = tile_begin[t + 1];
     u64 acc = scratch[t0 * kStreamMax + j];
-    for (int64_t tile = t0 + 1; tile < t1; ++tile) acc = fadd2(acc, scratch[tile * kStreamMax + j]);
+    // loads 16 tiles ahead of the (ordered) additions: the chain of adds is short, the chain of L2 latencies is not
+    for (int64_t tile = t0 + 1; tile < t1; tile += 16) {
+        u64 v[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) v[q] = (tile + q < t1) ? scratch[(tile + q) * kStreamMax + j] : 0ull;
+#pragma unroll
+        for (int q = 0; q < 16; ++q)
+            if (tile + q < t1) acc = fadd2(acc, v[q]);
+    }
     reinterpret_cast<u64*>(snr)[(int64_t)t * ld + j] = acc;
 }
 
