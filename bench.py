@@ -173,7 +173,7 @@ def run_ours(args):
     if args.path == 0 and L <= 64 and inp.n_filters >= (1 << 20):
         args.path = pkg.PATH_STREAM            # tiny chunks over a large bank: the HBM-bound streaming blocking
     opt = pkg.SpiirOptions(path=args.path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta,
-                           window_copies=args.window_copies)
+                           window_copies=args.window_copies, scan_segments=args.scan_segments)
     bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, local_rank, opt)
     x = torch.from_numpy(inp.x).cuda()
     keep_whole = (T * N * 8) <= args.max_snr_bytes
@@ -320,6 +320,7 @@ def main():
     ap.add_argument("--filters-per-thread", type=int, default=0)
     ap.add_argument("--warps-per-cta", type=int, default=0)
     ap.add_argument("--window-copies", type=int, default=0)
+    ap.add_argument("--scan-segments", type=int, default=0)
     ap.add_argument("--max-snr-bytes", type=float, default=20e9, help="keep the whole [T][N] SNR if it fits")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")

@@ -303,7 +303,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     if (path == SPIIR_PATH_SCAN || (path == SPIIR_PATH_AUTO && 2 * bk->n_items <= bk->n_sm && n >= 4 * kTS)) {
         const int64_t max_seg = std::max<int64_t>(1, n / kTS);
         int64_t want = bk->opt.scan_segments > 0 ? bk->opt.scan_segments
-                                                 : ((int64_t)2 * bk->n_sm + bk->n_items - 1) / bk->n_items;
+                                                 : ((int64_t)bk->n_sm + bk->n_items - 1) / bk->n_items;   // one wave of CTAs: longer segments amortise the window staging
         n_seg = std::min(std::max<int64_t>(want, 1), max_seg);
         if (n_seg < 2 && path != SPIIR_PATH_SCAN) n_seg = 1;
     }
