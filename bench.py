@@ -179,6 +179,8 @@ def run_ours(args):
     keep_whole = (T * N * 8) <= args.max_snr_bytes
     snr = torch.empty((T, N if keep_whole else L), dtype=torch.complex64, device="cuda")
     stream = torch.cuda.current_stream()
+    peak_power = torch.empty(T, dtype=torch.float32, device="cuda")
+    peak_index = torch.empty(T, dtype=torch.int32, device="cuda")
     n_calls = (N + L - 1) // L
 
     def one_step(events=None):
@@ -188,7 +190,10 @@ def run_ours(args):
                 events[i].record(stream)
             n = min(L, N - c0)
             out = snr[:, c0:c0 + n] if keep_whole else snr[:, :n]
-            pkg.spiir_filter(bank.handle, x[c0:c0 + n], out)
+            if args.peaks:
+                pkg.spiir_filter_peaks(bank.handle, x[c0:c0 + n], peak_power, peak_index, None if args.peaks == 1 else out)
+            else:
+                pkg.spiir_filter(bank.handle, x[c0:c0 + n], out)
         if events is not None:
             events[n_calls].record(stream)
 
@@ -262,7 +267,8 @@ def run_ours(args):
             "config": {"workload": workload_name(inp), "path": bank.last_path,
                        "l2": "each step writes %.2f GB of SNR and reads a %.0f MB bank: working set larger than the 126 MB L2"
                              % (T * N * 8 / 1e9, inp.n_filters * 28 / 1e6),
-                       "snr_buffer": "whole [T][N]" if keep_whole else "per-chunk [T][L] reused"},
+                       "snr_buffer": "whole [T][N]" if keep_whole else "per-chunk [T][L] reused",
+                       "entry": ["spiir_filter", "spiir_filter_peaks (no SNR output)", "spiir_filter_peaks (+ SNR output)"][args.peaks]},
             "pct_of_fp32_fma_peak": 100.0 * FLOPS_PER_FILTER_SAMPLE * value / world / (FP32_PEAK_TFLOPS * 1e12),
             "gpu_launches": int(launches), "roofline": roofline, "latency": latency, "clocks": clocks.summary()}
 
@@ -321,6 +327,7 @@ def main():
     ap.add_argument("--warps-per-cta", type=int, default=0)
     ap.add_argument("--window-copies", type=int, default=0)
     ap.add_argument("--scan-segments", type=int, default=0)
+    ap.add_argument("--peaks", type=int, default=0, help="1: spiir_filter_peaks without SNR output, 2: with (not the headline)")
     ap.add_argument("--max-snr-bytes", type=float, default=20e9, help="keep the whole [T][N] SNR if it fits")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")

@@ -90,6 +90,16 @@ int spiir_bank_create(spiir_bank **out, int32_t n_templates, const int64_t *filt
 int spiir_filter(spiir_bank *bank, const float *x_dev, int64_t n, float *snr_dev, int64_t ld,
                  void *stream);
 
+/* Filter the next n samples like spiir_filter and reduce them to one trigger candidate per template (SURVEY.md
+ * NEXT N4; "rapidly detect ... signals" -- the paper defines no trigger, reading Q16):
+ *   power_dev[t] = max over the n samples of this call of |SNR_t[j]|^2   (float32, computed from the FP32 SNR)
+ *   index_dev[t] = the first j in 0..n-1 that attains it
+ * Both DEVICE [T]; either may be NULL.  snr_dev may be NULL: then the series itself is not written (the only
+ * per-sample HBM traffic of the path disappears).  n >= 1.  The maximum is merged with integer atomic max
+ * over (power bits, index), so the result does not depend on the order of execution. */
+int spiir_filter_peaks(spiir_bank *bank, const float *x_dev, int64_t n, float *snr_dev, int64_t ld,
+                       float *power_dev, int32_t *index_dev, void *stream);
+
 /* Same operation with HOST buffers (the end-to-end entry): copies x to the device, filters, copies
  * SNR[t][0..n) back into snr_host (row stride ld), overlapping copies and kernels internally.
  * Buffers may be pageable or pinned.  Returns after the results are in snr_host. */

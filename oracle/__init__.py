@@ -120,6 +120,25 @@ def filter_outputs(a1, b0, delays, x) -> np.ndarray:
     return y
 
 
+def peaks(snr: np.ndarray, j0: int = 0, n: int | None = None):
+    """power[t] = max_j |snr[t, j0 + j]|^2 over j in [0, n), index[t] = first such j.  snr complex128 [T][N]."""
+    lib = _load()
+    snr = np.ascontiguousarray(snr, dtype=np.complex128)
+    T, N = snr.shape
+    n = N - j0 if n is None else n
+    if n < 1 or j0 < 0 or j0 + n > N:
+        raise ValueError("need 0 <= j0 and 1 <= n <= N - j0")
+    power = np.empty(T, dtype=np.float64)
+    index = np.empty(T, dtype=np.int64)
+    lib.spiir_oracle_peaks.restype = ctypes.c_int
+    rc = lib.spiir_oracle_peaks(ctypes.c_int32(T), _p(snr.view(np.float64), ctypes.c_double), ctypes.c_int64(N),
+                                ctypes.c_int64(j0), ctypes.c_int64(n), _p(power, ctypes.c_double),
+                                _p(index, ctypes.c_int64))
+    if rc != 0:
+        raise RuntimeError(f"spiir_oracle_peaks failed ({rc})")
+    return power, index
+
+
 class Stream:
     """Streaming oracle: state and the whole input past are carried across ``filter`` calls."""
 

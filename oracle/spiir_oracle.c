@@ -23,7 +23,8 @@
  *
  * Pins (tests/test_oracle_pins.py): impulse closed form, tone closed form with transient, brute-force
  * convolution, linearity/superposition, streaming == one-shot, a1 = 0 -> numpy.convolve,
- * d = 0 real pole -> scipy.signal.lfilter, exact dyadic golden vector, white-noise energy.
+ * d = 0 real pole -> scipy.signal.lfilter, exact dyadic golden vector, white-noise energy; spiir_oracle_peaks:
+ * single-filter impulse closed form (peak |b0|^2 at n0 + d) and numpy.argmax on random rows.
  * No function here is "parity unpinned".
  */
 #include <stdint.h>
@@ -188,6 +189,27 @@ int spiir_oracle_filter_outputs(int64_t K, const float *a1, const float *b0, con
             y[2 * (k * N + n)] = yre;
             y[2 * (k * N + n) + 1] = yim;
         }
+    }
+    return 0;
+}
+
+/* Trigger candidates (reading Q16 -- the paper only says the method should "rapidly
+ * detect ... signals", and defines no trigger): for every template t and the samples [j0, j0 + n) of
+ * its SNR row,  power[t] = max_j |SNR_t[j]|^2  and  index[t] = the first j - j0 that attains it.  Plain scan. */
+int spiir_oracle_peaks(int32_t T, const double *snr /* interleaved re, im */, int64_t ld, int64_t j0, int64_t n,
+                       double *power, int64_t *index)
+{
+    if (T < 0 || n < 1 || j0 < 0 || !snr || !power || !index) return -1;
+    for (int32_t t = 0; t < T; ++t) {
+        double best = -1.0;
+        int64_t arg = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            const double re = snr[2 * ((int64_t)t * ld + j0 + j)], im = snr[2 * ((int64_t)t * ld + j0 + j) + 1];
+            const double m = re * re + im * im;
+            if (m > best) { best = m; arg = j; }
+        }
+        power[t] = best;
+        index[t] = arg;
     }
     return 0;
 }

@@ -6,7 +6,7 @@ runs in the library's CUDA kernels.  There is no CPU fallback: without the built
 CUDA device the calls raise.
 """
 from .binding import (SpiirError, SpiirOptions, SpiirBank, spiir_bank_create, spiir_filter,  # noqa: F401
-                      spiir_filter_host, spiir_filter_host_async, spiir_bank_host_sync, spiir_bank_reset, spiir_bank_destroy, spiir_bank_num_templates,
+                      spiir_filter_peaks, spiir_filter_host, spiir_filter_host_async, spiir_bank_host_sync, spiir_bank_reset, spiir_bank_destroy, spiir_bank_num_templates,
                       spiir_bank_num_filters, spiir_bank_max_delay, spiir_bank_get_state,
                       spiir_bank_set_state, spiir_kernel_launches, spiir_last_error, spiir_version,
                       spiir_bank_last_path, spiir_layout_probe, shard_templates, load_library, library_path,

@@ -16,7 +16,7 @@ EXPORTS = ["spiir_bank_create", "spiir_filter", "spiir_filter_host", "spiir_bank
            "spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay",
            "spiir_bank_get_state", "spiir_bank_set_state", "spiir_bank_destroy", "spiir_last_error",
            "spiir_kernel_launches", "spiir_bank_last_path", "spiir_version", "spiir_layout_probe",
-           "spiir_filter_host_async", "spiir_bank_host_sync"]
+           "spiir_filter_host_async", "spiir_bank_host_sync", "spiir_filter_peaks"]
 
 
 class SpiirError(RuntimeError):
@@ -64,6 +64,8 @@ def load_library():
     lib.spiir_filter_host_async.argtypes = [vp, vp, i64, vp, i64]
     lib.spiir_bank_host_sync.restype = ctypes.c_int
     lib.spiir_bank_host_sync.argtypes = [vp]
+    lib.spiir_filter_peaks.restype = ctypes.c_int
+    lib.spiir_filter_peaks.argtypes = [vp, vp, i64, vp, i64, vp, vp, vp]
     lib.spiir_bank_reset.restype = ctypes.c_int
     lib.spiir_bank_reset.argtypes = [vp, vp]
     for name in ("spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay"):
@@ -135,6 +137,27 @@ def spiir_filter(bank, x, snr, ld: int | None = None, stream=None, n: int | None
         ld = int(snr.stride(0)) if snr.shape[0] > 1 else max(int(snr.shape[1]), n)
     _check(load_library().spiir_filter(bank, ctypes.c_void_p(x.data_ptr()), n, ctypes.c_void_p(snr.data_ptr()),
                                        int(ld), _stream_handle(stream)))
+
+
+def spiir_filter_peaks(bank, x, power=None, index=None, snr=None, stream=None):
+    """x: CUDA float32 [n]; power: CUDA float32 [T]; index: CUDA int32 [T]; snr: optional CUDA complex64 [T, >=n]."""
+    import torch
+    if x.dtype != torch.float32 or not x.is_cuda or not x.is_contiguous():
+        raise ValueError("x must be a contiguous CUDA float32 tensor")
+    for name, t, dt in (("power", power, torch.float32), ("index", index, torch.int32)):
+        if t is not None and (t.dtype != dt or not t.is_cuda or not t.is_contiguous()):
+            raise ValueError(f"{name} must be a contiguous CUDA {dt} tensor")
+    n, ld, snr_ptr = int(x.numel()), int(x.numel()), None
+    if snr is not None:
+        if snr.dtype != torch.complex64 or not snr.is_cuda or snr.dim() != 2 or snr.shape[1] < n or \
+                (snr.shape[1] > 1 and snr.stride(1) != 1):
+            raise ValueError("snr must be a CUDA complex64 [T, >=n] tensor with unit column stride")
+        ld = int(snr.stride(0)) if snr.shape[0] > 1 else max(int(snr.shape[1]), n)
+        snr_ptr = ctypes.c_void_p(snr.data_ptr())
+    _check(load_library().spiir_filter_peaks(bank, ctypes.c_void_p(x.data_ptr()), n, snr_ptr, ld,
+                                             ctypes.c_void_p(power.data_ptr()) if power is not None else None,
+                                             ctypes.c_void_p(index.data_ptr()) if index is not None else None,
+                                             _stream_handle(stream)))
 
 
 def spiir_filter_host(bank, x: np.ndarray, snr: np.ndarray | None = None, asynchronous: bool = False) -> np.ndarray:

@@ -57,7 +57,7 @@ struct spiir_bank {
     int F = 8, W = 16, NC = 1;
     bool uniform_groups = true;
     bool gmem_only = false;          // the history alone exceeds shared memory: x is read through L1/L2
-    bool configured[2] = {false, false};
+    bool configured[2][2] = {{false, false}, {false, false}};
     int64_t T = 0, K = 0, D = 0, n_slots = 0, n_tiles = 0;
     int32_t n_items = 0;
     double avg_conflict_degree = 0.0;
@@ -70,6 +70,10 @@ struct spiir_bank {
     int64_t* tile_begin = nullptr;   // [T+1] first warp tile of every template (streaming combine)
     u64* stream_scratch = nullptr;   // [n_tiles][kStreamMax] per-tile partial sums (streaming path)
     bool stream_configured = false;
+    u64* peaks = nullptr;            // [T] packed (power bits << 32 | ~index) of the running call (spiir_filter_peaks)
+    float* peak_snr = nullptr;       // internal SNR rows for spiir_filter_peaks without an SNR buffer (multi-round templates)
+    int64_t peak_snr_cap = 0;
+    bool multi_round = false;        // some template spans several CTA rounds (its sums accumulate through the SNR rows)
     WarpWork* work = nullptr;
     int64_t* slot_of_filter = nullptr;
     // input tape: tape[cur][0..pos) holds the most recent samples, the next chunk is appended at pos
@@ -107,7 +111,7 @@ void free_bank(spiir_bank* bk)
 {
     if (!bk) return;
     cudaFree(bk->ar); cudaFree(bk->ai2); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
-    cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->tile_begin); cudaFree(bk->stream_scratch); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
+    cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->tile_begin); cudaFree(bk->stream_scratch); cudaFree(bk->peaks); cudaFree(bk->peak_snr); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
     cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
     cudaFree(bk->hx); cudaFree(bk->hsnr[0]); cudaFree(bk->hsnr[1]);
     for (int i = 0; i < 2; ++i) {
@@ -158,14 +162,17 @@ int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
 // The compiled (F, W) register/warp blockings of the filter kernel: F filters per thread, W warps per CTA.
 // W is chosen so that the register file of an SM is full with one resident CTA (the shared-memory window of
 // a 16 384-sample chunk behind a 16 383-sample history allows only one).
-const void* select_kernel(int F, int W, int NC, bool g)
+const void* select_kernel(int F, int W, int NC, bool g, bool peak = false)
 {
+#define SPIIR_VARIANT_P(F_, W_, M_, P_)                                                        \
+        if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true, M_, P_>;               \
+        if (NC == 4) return (const void*)spiir_filter_kernel<F_, W_, 4, false, M_, P_>;        \
+        if (NC == 2) return (const void*)spiir_filter_kernel<F_, W_, 2, false, M_, P_>;        \
+        return (const void*)spiir_filter_kernel<F_, W_, 1, false, M_, P_>;
 #define SPIIR_VARIANT(F_, W_, M_)                                                              \
     if (F == F_ && W == W_) {                                                                  \
-        if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true, M_>;                   \
-        if (NC == 4) return (const void*)spiir_filter_kernel<F_, W_, 4, false, M_>;            \
-        if (NC == 2) return (const void*)spiir_filter_kernel<F_, W_, 2, false, M_>;            \
-        return (const void*)spiir_filter_kernel<F_, W_, 1, false, M_>;                         \
+        if (peak) { SPIIR_VARIANT_P(F_, W_, M_, true) }                                        \
+        SPIIR_VARIANT_P(F_, W_, M_, false)                                                     \
     }
     SPIIR_VARIANT(16, 8, 1)
     SPIIR_VARIANT(8, 8, 2)
@@ -175,6 +182,7 @@ const void* select_kernel(int F, int W, int NC, bool g)
     SPIIR_VARIANT(4, 32, 1)
     SPIIR_VARIANT(2, 32, 1)
 #undef SPIIR_VARIANT
+#undef SPIIR_VARIANT_P
     return nullptr;
 }
 
@@ -188,13 +196,13 @@ int part_buffers(int F, int W) { return (W == 8 && (F == 8 || F == 4)) ? 2 : kPB
 size_t fixed_smem(int F, int W) { return filter_smem_bytes(W, 1, 0, true, nullptr, part_buffers(F, W)); }
 
 // allow the kernel to use all opt-in shared memory (once per variant and bank)
-int configure_kernel(spiir_bank* bk, bool g, const void** fn)
+int configure_kernel(spiir_bank* bk, bool g, const void** fn, bool peak = false)
 {
-    *fn = select_kernel(bk->F, bk->W, bk->NC, g);
+    *fn = select_kernel(bk->F, bk->W, bk->NC, g, peak);
     if (!*fn) return fail(SPIIR_EINVAL, "unsupported blocking F=%d W=%d", bk->F, bk->W);
-    if (!bk->configured[g]) {
+    if (!bk->configured[g][peak]) {
         CU_TRY(cudaFuncSetAttribute(*fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bk->smem_optin));
-        bk->configured[g] = true;
+        bk->configured[g][peak] = true;
     }
     return SPIIR_OK;
 }
@@ -202,7 +210,7 @@ int configure_kernel(spiir_bank* bk, bool g, const void** fn)
 int launch_filter(spiir_bank* bk, bool g, const FilterParams& p, dim3 grid, size_t smem, cudaStream_t st)
 {
     const void* fn = nullptr;
-    int rc = configure_kernel(bk, g, &fn);
+    int rc = configure_kernel(bk, g, &fn, p.peaks != nullptr);     // the trigger reduction is a variant of its own
     if (rc) return rc;
     void* args[] = {(void*)&p};
     CU_TRY(cudaLaunchKernel(fn, grid, dim3((unsigned)(kWarp * bk->W), 1, 1), args, smem, st));
@@ -255,7 +263,7 @@ const void* select_stream_kernel(int F, int NC)
     return nullptr;
 }
 
-int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st)
+int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st, u64* peaks)
 {
     const void* fn = select_stream_kernel(bk->F, bk->NC);
     if (!fn) return fail(SPIIR_EINVAL, "no streaming kernel for F=%d NC=%d", bk->F, bk->NC);
@@ -278,7 +286,7 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
     CU_TRY(cudaLaunchKernel(fn, dim3((unsigned)ctas, 1, 1), dim3(kWarp * kStreamWarps, 1, 1), args, smem, st));
     const int64_t total = bk->T * n;
     spiir_stream_combine_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(bk->stream_scratch, bk->tile_begin,
-                                                                             (int32_t)bk->T, (int32_t)n, snr, ld);
+                                                                             (int32_t)bk->T, (int32_t)n, snr, ld, peaks);
     g_launches.fetch_add(2, std::memory_order_relaxed);
     CU_TRY(cudaGetLastError());
     bk->last_path = SPIIR_PATH_STREAM;
@@ -286,7 +294,7 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
 }
 
 // Run the filter kernels over n samples whose window starts at xwin (aligned), sample 0 at xwin[w0].
-int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st)
+int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st, u64* peaks)
 {
     const size_t smem_cap = bk->smem_optin;
     // window floats per copy that fit beside the reduction buffers (a copy is padded by up to 47 floats)
@@ -295,7 +303,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     int path = bk->opt.path;
     if (path == SPIIR_PATH_STREAM && n <= kStreamMax && !gmem && select_stream_kernel(bk->F, bk->NC) &&
         stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr) <= smem_cap)
-        return run_stream(bk, xwin, w0, n, snr, ld, st);
+        return run_stream(bk, xwin, w0, n, snr, ld, st, peaks);
     // ---- how much time-parallelism is needed to fill the machine?  The scan path does the recurrence twice, so it
     // only pays when the bank leaves at least half of the SMs idle (cfg2: 128 items on 148 SMs run 1.7x faster
     // sequentially).
@@ -321,7 +329,8 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
             FilterParams p = base_params(bk);
             p.y_in = bk->y; p.y_out = bk->y; p.y_in_stride = 0; p.y_out_stride = 0; p.store_last_only = 1;
             p.xwin = xwin + off; p.w0 = w0; p.n = ns; p.seg_len = ns;
-            p.snr = snr + 2 * off; p.ld = ld;
+            p.snr = snr ? snr + 2 * off : nullptr; p.ld = ld;
+            p.peaks = peaks; p.peak_off = off;
             const size_t smem = filter_smem_bytes(bk->W, bk->NC, w0 + ns, gmem, nullptr, part_buffers(bk->F, bk->W));
             int occ = 1;
             int rc = cached_occupancy(bk, gmem, smem, &occ);
@@ -378,6 +387,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
         p.y_in = bk->cbuf; p.y_in_stride = 2 * bk->n_slots; p.y_out = bk->y; p.y_out_stride = 0; p.store_last_only = 1;
         p.xwin = xwin; p.w0 = w0; p.n = n; p.seg_len = seg_len;
         p.snr = snr; p.ld = ld;
+        p.peaks = peaks; p.peak_off = 0;
         dim3 grid(gx, (unsigned)n_seg, 1);
         rc = launch_filter(bk, gmem, p, grid, smem, st);
         if (rc) return rc;
@@ -538,6 +548,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->n_items = (int32_t)(L.item_round0.size() - 1);
     bk->avg_conflict_degree = L.avg_conflict_degree;
     bk->uniform_groups = L.uniform_groups;
+    bk->multi_round = (L.work.size() / (size_t)bk->W) > (L.item_round0.size() - 1);
     if (e == cudaSuccess) e = upload(&bk->ar, L.ar);
     if (e == cudaSuccess) e = upload(&bk->ai2, L.ai2);
     if (e == cudaSuccess) e = upload(&bk->b, L.b);
@@ -563,6 +574,26 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     return SPIIR_OK;
 }
 
+namespace {
+
+// spiir_filter and spiir_filter_peaks: append the chunk to the tape, run the kernels, advance the tape.
+int filter_impl(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, int64_t ld, cudaStream_t st, u64* peaks)
+{
+    CU_TRY(cudaSetDevice(bk->device));
+    int rc = ensure_tape(bk, n, st);
+    if (rc) return rc;
+    float* tape = bk->tape[bk->cur];
+    CU_TRY(cudaMemcpyAsync(tape + bk->pos, x_dev, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    const int64_t start_al = (bk->pos - bk->D) / 4 * 4;
+    const int w0 = (int)(bk->pos - start_al);
+    rc = run_chunk(bk, tape + start_al, w0, n, snr_dev, ld, st, peaks);
+    if (rc) { bk->poisoned = true; return rc; }
+    bk->pos += n;
+    return SPIIR_OK;
+}
+
+}  // namespace
+
 int spiir_filter(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, int64_t ld, void* stream)
 {
     if (!bk) return fail(SPIIR_EINVAL, "null bank");
@@ -571,17 +602,38 @@ int spiir_filter(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, 
     if (n == 0) return SPIIR_OK;
     if (!x_dev || !snr_dev) return fail(SPIIR_EINVAL, "null device pointer");
     if (n > (int64_t)1 << 30) return fail(SPIIR_EINVAL, "chunk too long");
+    return filter_impl(bk, x_dev, n, snr_dev, ld, (cudaStream_t)stream, nullptr);
+}
+
+int spiir_filter_peaks(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, int64_t ld, float* power_dev,
+                       int32_t* index_dev, void* stream)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    if (bk->poisoned) return fail(SPIIR_ESTATE, "bank unusable after an earlier failure");
+    if (n < 1) return fail(SPIIR_EINVAL, "need n >= 1 (a peak over no samples is undefined)");
+    if (snr_dev && ld < n) return fail(SPIIR_EINVAL, "need n <= ld");
+    if (!x_dev || (!power_dev && !index_dev)) return fail(SPIIR_EINVAL, "null device pointer");
+    if (n > (int64_t)1 << 30) return fail(SPIIR_EINVAL, "chunk too long");
     cudaStream_t st = (cudaStream_t)stream;
     CU_TRY(cudaSetDevice(bk->device));
-    int rc = ensure_tape(bk, n, st);
+    if (!bk->peaks) CU_TRY(cudaMalloc((void**)&bk->peaks, (size_t)bk->T * sizeof(u64)));
+    if (!snr_dev && bk->multi_round) {
+        // templates that span several CTA rounds accumulate their sums through SNR rows: give them private ones
+        if (bk->peak_snr_cap < bk->T * n) {
+            CU_TRY(cudaStreamSynchronize(st));
+            cudaFree(bk->peak_snr); bk->peak_snr = nullptr; bk->peak_snr_cap = 0;
+            CU_TRY(cudaMalloc((void**)&bk->peak_snr, (size_t)bk->T * n * 2 * sizeof(float)));
+            bk->peak_snr_cap = bk->T * n;
+        }
+        snr_dev = bk->peak_snr;
+        ld = n;
+    }
+    CU_TRY(cudaMemsetAsync(bk->peaks, 0, (size_t)bk->T * sizeof(u64), st));
+    int rc = filter_impl(bk, x_dev, n, snr_dev, snr_dev ? ld : n, st, bk->peaks);
     if (rc) return rc;
-    float* tape = bk->tape[bk->cur];
-    CU_TRY(cudaMemcpyAsync(tape + bk->pos, x_dev, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st));
-    const int64_t start_al = (bk->pos - bk->D) / 4 * 4;
-    const int w0 = (int)(bk->pos - start_al);
-    rc = run_chunk(bk, tape + start_al, w0, n, snr_dev, ld, st);
-    if (rc) { bk->poisoned = true; return rc; }
-    bk->pos += n;
+    spiir_unpack_peaks_kernel<<<(unsigned)((bk->T + 255) / 256), 256, 0, st>>>(bk->peaks, power_dev, index_dev, (int32_t)bk->T);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CU_TRY(cudaGetLastError());
     return SPIIR_OK;
 }
 

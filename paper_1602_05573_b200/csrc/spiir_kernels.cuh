@@ -63,8 +63,12 @@ struct FilterParams {
     int64_t n;              // samples in this launch
     int64_t seg_len;        // samples per segment (multiple of kTS unless single segment)
     // output
-    float* snr;             // complex64 rows, nullptr = no output (carry pass)
+    float* snr;             // complex64 rows; nullptr with peaks == nullptr = no sums at all (carry pass)
     int64_t ld;             // row stride in complex elements
+    // fused trigger reduction: peaks[t] = max over this call of (bits(|SNR_t[n]|^2) << 32 | ~n),
+    // merged with atomicMax (order independent -> deterministic); nullptr = off
+    u64* peaks;
+    int64_t peak_off;       // index of this launch's first sample within the call
 };
 
 // One register tile: advance F filters by NV <= 8 samples, S[j] = sum over the thread's filters.
@@ -165,15 +169,56 @@ __device__ __forceinline__ void mbar_wait(u64* bar, unsigned parity)
 
 // Sum the partial rows of the warps of one template for ns samples and store them (fixed order over warps).
 // The ns samples are shared out over the lanes of the template's warps.
-template <int TS>
-__device__ __forceinline__ void cross_warp_store(const u64* __restrict__ pb, const WarpWork& ww, int warp, int lane, int ns,
-                                                 u64* __restrict__ out, bool accumulate)
+// |z|^2 and the sample index packed so that an unsigned max picks the largest power and, among equals, the earliest
+// sample (powers are non-negative floats: their bit patterns order like unsigned integers).
+__device__ __forceinline__ u64 peak_key(u64 z, int64_t idx)
 {
-    for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
-        u64 acc = pb[(size_t)ww.first * TS + s];
-        for (int w = 1; w < ww.count; ++w) acc = fadd2(acc, pb[(size_t)(ww.first + w) * TS + s]);
-        if (accumulate) acc = fadd2(out[s], acc);
-        out[s] = acc;
+    float re, im;
+    unpack2(z, re, im);
+    const float m = fmaf(re, re, im * im);
+    return ((u64)__float_as_uint(m) << 32) | (u64)(0xffffffffu - (unsigned)idx);
+}
+
+__device__ __forceinline__ void peak_commit(u64 best, u64* __restrict__ slot)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        const u64 o = __shfl_xor_sync(0xffffffffu, best, d);
+        best = o > best ? o : best;
+    }
+    if ((threadIdx.x & 31) == 0 && best) atomicMax(slot, best);
+}
+
+// Sum the partial rows of the warps of one template for ns samples and store them (fixed order over warps).
+// The ns samples are shared out over the lanes of the template's warps.  out == nullptr: no SNR output;
+// peak != nullptr: fold |SNR|^2 of these samples (call indices idx0 ..) into the template's peak.
+template <int TS, bool PEAK>
+__device__ __forceinline__ void cross_warp_store(const u64* __restrict__ pb, const WarpWork& ww, int warp, int lane, int ns,
+                                                 u64* __restrict__ out, bool accumulate, u64* __restrict__ peak = nullptr,
+                                                 int64_t idx0 = 0)
+{
+    if constexpr (!PEAK) {
+        for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
+            u64 acc = pb[(size_t)ww.first * TS + s];
+            for (int w = 1; w < ww.count; ++w) acc = fadd2(acc, pb[(size_t)(ww.first + w) * TS + s]);
+            if (accumulate) acc = fadd2(out[s], acc);
+            out[s] = acc;
+        }
+    } else {
+        u64 best = 0ull;
+        for (int s = lane + kWarp * (warp - ww.first); s < ns; s += kWarp * ww.count) {
+            u64 acc = pb[(size_t)ww.first * TS + s];
+            for (int w = 1; w < ww.count; ++w) acc = fadd2(acc, pb[(size_t)(ww.first + w) * TS + s]);
+            if (out) {
+                if (accumulate) acc = fadd2(out[s], acc);
+                out[s] = acc;
+            }
+            if (peak) {
+                const u64 k = peak_key(acc, idx0 + s);
+                best = k > best ? k : best;
+            }
+        }
+        if (peak) peak_commit(best, peak);
     }
 }
 
@@ -193,7 +238,8 @@ __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_l
 // Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
 // MINB = CTAs the register allocation must leave room for on one SM (tiny-chunk streaming: several small CTAs
 // per SM overlap one CTA's coefficient loads with another's arithmetic).
-template <int F, int W, int NC, bool GMEM_X, int MINB = 1>
+// PEAK compiles the fused trigger reduction in (spiir_filter_peaks); the plain kernel is untouched by it.
+template <int F, int W, int NC, bool GMEM_X, int MINB = 1, bool PEAK = false>
 __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const FilterParams p)
 {
     static_assert(!GMEM_X || NC == 1, "the global-memory window variant reads scalars");
@@ -239,7 +285,8 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     u64* bars = part64 + (size_t)(kAsync ? kPB : 2) * W * TS;                                // [W][kPB], indexed by a group's first warp
     u64* mytr = trbuf + (size_t)warp * kTrWarp;
     // per-template hand-over without any CTA-wide barrier: only where one CTA owns the SM and all rounds have one shape
-    const bool async = kAsync && p.uniform_groups && p.snr;
+    const bool sums = PEAK ? (p.snr || p.peaks) : (p.snr != nullptr);                                        // false: carry pass, states only
+    const bool async = kAsync && p.uniform_groups && sums;
     if (async && tid < W) {
         const int first = p.canon[2 * tid], count = p.canon[2 * tid + 1];
         if (first == tid && count > 0)
@@ -273,7 +320,10 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                 }
             }
             const bool accumulate = (r > r0);
-            u64* const out_row = reinterpret_cast<u64*>(p.snr) + (int64_t)ww.row * p.ld + t0;
+            u64* const out_row = (!PEAK || p.snr) ? reinterpret_cast<u64*>(p.snr) + (int64_t)ww.row * p.ld + t0 : nullptr;
+            // multi-round templates: only the last round sees the complete sums
+            u64* const peak = (PEAK && p.peaks && active && r == r1 - 1) ? p.peaks + ww.row : nullptr;
+            const int64_t idx_row = p.peak_off + t0;
             if (async) {
                 if (active) {
                     int prev_ns = 0;
@@ -296,7 +346,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                         // finish the previous super tile before announcing this one (keeps 3 buffers sufficient)
                         if (prev_ns) {
                             mbar_wait(mybars + prev_use % kPB, (prev_use / kPB) & 1);
-                            cross_warp_store<TS>(part64 + (size_t)(prev_use % kPB) * W * TS, ww, warp, lane, prev_ns, out_row + prev_st, accumulate);
+                            cross_warp_store<TS, PEAK>(part64 + (size_t)(prev_use % kPB) * W * TS, ww, warp, lane, prev_ns, (!PEAK || out_row) ? out_row + prev_st : nullptr, accumulate, peak, idx_row + prev_st);
                         }
                         __syncwarp();
                         if (lane == 0) mbar_arrive(mybars + i % kPB);
@@ -304,7 +354,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                     }
                     if (prev_ns) {
                         mbar_wait(mybars + prev_use % kPB, (prev_use / kPB) & 1);
-                        cross_warp_store<TS>(part64 + (size_t)(prev_use % kPB) * W * TS, ww, warp, lane, prev_ns, out_row + prev_st, accumulate);
+                        cross_warp_store<TS, PEAK>(part64 + (size_t)(prev_use % kPB) * W * TS, ww, warp, lane, prev_ns, (!PEAK || out_row) ? out_row + prev_st : nullptr, accumulate, peak, idx_row + prev_st);
                     }
                 }
             } else {
@@ -319,16 +369,16 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                             const int nv = ns - tt;
                             if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
                             else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
-                            if (p.snr) {
+                            if (sums) {
                                 const u64 P = warp_reduce_tile(S, mytr, lane);
                                 if (lane < kTT) mypart[tt + lane] = P;
                             }
                         }
                     }
-                    if (p.snr) {
+                    if (sums) {
                         __syncthreads();
                         if (active)
-                            cross_warp_store<TS>(part64 + (size_t)buf * W * TS, ww, warp, lane, ns, out_row + st, accumulate);
+                            cross_warp_store<TS, PEAK>(part64 + (size_t)buf * W * TS, ww, warp, lane, ns, (!PEAK || out_row) ? out_row + st : nullptr, accumulate, peak, idx_row + st);
                     }
                 }
             }
@@ -340,7 +390,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                     *reinterpret_cast<u64*>(yo + 2 * s) = Y[f];
                 }
             }
-            if (p.snr && !async) __syncthreads();      // part rows are rewritten in the next round
+            if (sums && !async) __syncthreads();      // part rows are rewritten in the next round
         }
     }
 }
@@ -453,7 +503,8 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
 
 // SNR[t][j] = sum over the warp tiles of template t, in tile order, of scratch[tile][j].  One thread per (t, j).
 __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, const int64_t* __restrict__ tile_begin,
-                                            int32_t n_templates, int32_t n, float* __restrict__ snr, int64_t ld)
+                                            int32_t n_templates, int32_t n, float* __restrict__ snr, int64_t ld,
+                                            u64* __restrict__ peaks)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= (int64_t)n_templates * n) return;
@@ -469,7 +520,8 @@ __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, con
         for (int q = 0; q < 16; ++q)
             if (tile + q < t1) acc = fadd2(acc, v[q]);
     }
-    reinterpret_cast<u64*>(snr)[(int64_t)t * ld + j] = acc;
+    if (snr) reinterpret_cast<u64*>(snr)[(int64_t)t * ld + j] = acc;
+    if (peaks) atomicMax(peaks + t, peak_key(acc, j));
 }
 
 // ---- time-parallel scan: carry combine.  For every slot, given the carried state c_0 = y and the
@@ -518,6 +570,16 @@ __global__ void spiir_scan_carry_kernel(const float* __restrict__ ar, const floa
 }
 
 // ---- small utilities
+__global__ void spiir_unpack_peaks_kernel(const u64* __restrict__ peaks, float* __restrict__ power, int32_t* __restrict__ arg,
+                                          int32_t n_templates)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_templates) return;
+    const u64 k = peaks[t];
+    if (power) power[t] = __uint_as_float((unsigned)(k >> 32));
+    if (arg) arg[t] = (int32_t)(0xffffffffu - (unsigned)(k & 0xffffffffu));
+}
+
 __global__ void spiir_permute_state_kernel(const float* __restrict__ src, float* __restrict__ dst,
                                            const int64_t* __restrict__ slot_of_filter, int64_t K, int to_slots)
 {

@@ -216,6 +216,17 @@ def test_cfg4_tiny_chunks(env, path):
     check(got, ref)
 
 
+def test_cfg4_full_bank_in_bench_configuration(env):
+    # the whole 8192-template bank (4.7 M filters), streaming blocking and 16-sample calls exactly as bench.py --config 4
+    # runs it; 64 calls, sampled templates stratified over the filter count
+    inp = spiir_inputs.make_config(4, n_samples=1024)
+    kt = np.diff(inp.offsets)
+    rows = np.sort(np.argsort(kt)[np.linspace(0, inp.n_templates - 1, 12).astype(int)])
+    ref = env[1].run_inputs(inp.select_templates(rows))
+    got = run_gpu(env, inp, chunks=[16] * 64, path=3, rows=rows)
+    check(got, ref)
+
+
 def test_mixed_template_sizes_over_many_cta_items(env):
     # more CTA items than SMs, every item a different mix of template sizes: CTAs walk through several items whose
     # warp groups differ (regression: named barriers shared between groups of different shape)
@@ -306,3 +317,67 @@ def test_reset_and_host_entry(env):
         second = bank.filter(x).cpu().numpy()
     assert np.array_equal(first.view(np.float32), second.view(np.float32))
     check(first, ref)
+
+
+# ------------------------------------------------------------------ fused trigger reduction (spiir_filter_peaks)
+def check_peaks(pkg, torch, oracle, inp, chunks, opt, with_snr, ref):
+    """GPU power/index per call against the oracle: the power within tolerance; the index must point at a sample whose
+    oracle power is within tolerance of the oracle maximum (several indices are correct when powers nearly tie)."""
+    T = inp.n_templates
+    x = torch.from_numpy(inp.x).cuda()
+    power = torch.empty(T, dtype=torch.float32, device="cuda")
+    index = torch.empty(T, dtype=torch.int32, device="cuda")
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank:
+        pos = 0
+        for c in chunks:
+            snr = torch.full((T, c), float("nan"), dtype=torch.complex64, device="cuda") if with_snr else None
+            pkg.spiir_filter_peaks(bank.handle, x[pos:pos + c], power, index, snr)
+            torch.cuda.synchronize()
+            p_ref, i_ref = oracle.peaks(ref, pos, c)
+            p, i = power.cpu().numpy().astype(np.float64), index.cpu().numpy().astype(np.int64)
+            scale = (np.abs(ref).max(axis=1)) ** 2
+            assert np.all((i >= 0) & (i < c))
+            assert np.all(np.abs(p - p_ref) <= 4e-4 * scale), (np.abs(p - p_ref) / scale).max()
+            at = np.abs(ref[np.arange(T), pos + i]) ** 2
+            assert np.all(p_ref - at <= 4e-4 * scale)
+            if with_snr:
+                got = snr.cpu().numpy()
+                assert np.isfinite(got.view(np.float32)).all()
+                m = got.real.astype(np.float32) ** 2 + got.imag.astype(np.float32) ** 2      # the kernel's own decision
+                assert np.allclose(p, m.max(axis=1), rtol=1e-6)
+            pos += c
+
+
+@pytest.mark.parametrize("path,with_snr", [(1, True), (1, False), (2, True), (3, False), (3, True)])
+def test_filter_peaks_against_oracle(env, path, with_snr):
+    pkg, oracle, torch = env
+    inp = spiir_inputs.make_random_bank(51, [256, 100, 512, 33, 1024, 64, 5000, 700], 4096 + 300, d_max=700)
+    ref = oracle.run_inputs(inp)
+    chunks = [2048, 300, 2048] if path != 3 else [64, 16, 1, 40] + [64] * 66
+    chunks = chunks[:] if sum(chunks) <= inp.n_samples else chunks
+    assert sum(chunks) <= inp.n_samples
+    check_peaks(pkg, torch, oracle, inp, chunks, pkg.SpiirOptions(path=path), with_snr, ref)
+
+
+def test_filter_peaks_cfg3_blocking_and_exact_tie(env):
+    pkg, oracle, torch = env
+    inp = spiir_inputs.make_config(3, n_templates=8, n_samples=16384)
+    ref = oracle.run_inputs(inp)
+    check_peaks(pkg, torch, oracle, inp, [16384], pkg.SpiirOptions(path=1), False, ref)
+    # exact arithmetic (dyadic golden bank): two equal maxima -> the earlier index, bit-exact power
+    off = np.array([0, 1], np.int64)
+    a1, b0, d = np.array([0.0], np.complex64), np.array([1.0 + 0j], np.complex64), np.array([0], np.int32)
+    xs = np.zeros(100, np.float32)
+    xs[17] = xs[60] = 3.0
+    xs[40] = -2.0
+    x = torch.from_numpy(xs).cuda()
+    power = torch.empty(1, dtype=torch.float32, device="cuda")
+    index = torch.empty(1, dtype=torch.int32, device="cuda")
+    for path in (1, 2, 3):
+        with pkg.SpiirBank(off, a1, b0, d, 0, pkg.SpiirOptions(path=path)) as bank:
+            pkg.spiir_filter_peaks(bank.handle, x[:64], power, index)
+            torch.cuda.synchronize()
+            assert power.item() == 9.0 and index.item() == 17
+            pkg.spiir_filter_peaks(bank.handle, x[64:], power, index)
+            torch.cuda.synchronize()
+            assert power.item() == 0.0 and index.item() == 0

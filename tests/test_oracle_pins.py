@@ -245,3 +245,29 @@ def test_generators_are_seeded_and_in_range():
         assert np.abs(c.a1.astype(np.complex128)).max() < 1.0
     sub = c1.select_templates([3, 0])
     assert np.array_equal(sub.a1[:256], c1.a1[768:]) and np.array_equal(sub.a1[256:], c1.a1[:256])
+
+
+# ------------------------------------------------------------------ trigger candidates
+def test_peaks_impulse_closed_form():
+    # one filter, impulse at n0: |y[n]|^2 = |b0|^2 |a1|^(2(n - n0 - d)) decays from its first non-zero sample, so the
+    # peak is |b0|^2 at n0 + d (north_star impulse response); a window that starts later sees its first sample largest
+    a1, b0, d, n0, N = 0.9 * np.exp(0.3j), 0.5 - 0.25j, 7, 11, 64
+    x = np.zeros(N, np.float32)
+    x[n0] = 1.0
+    snr = oracle.run(np.array([0, 1]), np.array([a1], np.complex64), np.array([b0], np.complex64), np.array([d], np.int32), x)
+    p, i = oracle.peaks(snr)
+    assert i[0] == n0 + d and p[0] == pytest.approx(abs(np.complex64(b0)) ** 2, rel=1e-12)
+    p2, i2 = oracle.peaks(snr, j0=30, n=20)
+    assert i2[0] == 0 and p2[0] == pytest.approx(abs(np.complex64(b0)) ** 2 * abs(np.complex64(a1)) ** (2 * (30 - n0 - d)), rel=1e-6)
+
+
+def test_peaks_match_numpy_argmax_and_take_the_first_of_equals():
+    rng = np.random.default_rng(3)
+    snr = rng.standard_normal((9, 200)) + 1j * rng.standard_normal((9, 200))
+    snr[4, 50] = snr[4, 120] = 30.0 + 40.0j                       # a tie: the earlier sample wins
+    for j0, n in ((0, 200), (13, 57), (199, 1)):
+        p, i = oracle.peaks(snr, j0, n)
+        m = np.abs(snr[:, j0:j0 + n]) ** 2
+        assert np.array_equal(i, m.argmax(axis=1))
+        assert np.allclose(p, m.max(axis=1), rtol=1e-14)
+    assert oracle.peaks(snr)[1][4] == 50
