@@ -399,14 +399,15 @@ int choose_F(int32_t T, const int64_t* off, int requested)
 {
     if (requested == 2 || requested == 4 || requested == 8 || requested == 16) return requested;
     // Least padded work, weighted by the measured speed of the inner loops on a padding-free bank (cfg3:
-    // F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 / 32 warps 44 % of FP32 peak).
+    // F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 / 32 warps 44 %, F = 2 / 32 warps 33 % of FP32 peak).
+    // F = 2 (64-filter warp tiles) only wins for banks of very small templates (PAPER.md:L335 maps those to one warp).
     double best = 0;
     int bestF = 0;
-    for (int F : {16, 8, 4}) {
+    for (int F : {16, 8, 4, 2}) {
         const int64_t per = 32LL * F;
         double padded = 0;
         for (int32_t t = 0; t < T; ++t) padded += (double)((off[t + 1] - off[t] + per - 1) / per * per);
-        padded *= (F == 16 ? 1.0 : (F == 8 ? 1.05 : 1.22));
+        padded *= (F == 16 ? 1.0 : (F == 8 ? 1.05 : (F == 4 ? 1.22 : 1.63)));
         if (!bestF || padded < best) { best = padded; bestF = F; }
     }
     return bestF;

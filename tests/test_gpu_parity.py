@@ -140,6 +140,17 @@ def test_ragged_templates_all_register_blockings(env, F):
     check(run_gpu(env, inp, chunks=[500, 9, 991], path=2, F=F, segments=5), ref)
 
 
+def test_bank_of_very_small_templates(env):
+    # PAPER.md:L335 maps templates of <= 32 filters to one warp; here they are padded to the smallest warp tile
+    # (the bank picks F = 2 by itself) -- correct, not yet efficient (DESIGN.md NEXT N1)
+    counts = [32, 17, 8, 1, 32, 30, 2, 25] * 40
+    inp = spiir_inputs.make_random_bank(61, counts, 900, d_max=400)
+    rows = np.arange(0, len(counts), 13)
+    ref = env[1].run_inputs(inp.select_templates(rows))
+    check(run_gpu(env, inp, chunks=[400, 500], rows=rows), ref)
+    check(run_gpu(env, inp, chunks=[64] * 14 + [4], path=3, rows=rows), ref)
+
+
 def test_zero_delay_and_constant_delay(env):
     rng = np.random.default_rng(5)
     inp = spiir_inputs.make_random_bank(6, [128, 40], 700, d_max=0)
