@@ -51,13 +51,16 @@ enum {
 typedef struct spiir_options {
     int32_t struct_size;        /* = sizeof(spiir_options); lets the struct grow compatibly */
     int32_t path;               /* SPIIR_PATH_*; default AUTO */
-    int32_t filters_per_thread; /* 0 = choose; else 2, 4, 8 or 16 (register blocking of the throughput kernel) */
+    int32_t filters_per_thread; /* 0 = choose; else 1, 2, 4, 8 or 16 (register blocking of the throughput kernel) */
     int32_t scan_segments;      /* 0 = choose; else time segments per call for SPIIR_PATH_SCAN */
     int32_t warps_per_cta;      /* 0 = choose; else 8, 16 or 32; valid (filters_per_thread, warps_per_cta) pairs:
-                                   (16,8) (8,8) (8,16) (4,8) (4,16) (4,32) (2,32) */
+                                   (16,8) (8,8) (8,16) (4,8) (4,16) (4,32) (2,32) (1,32) */
     int32_t window_copies;      /* 0 = choose; else 1, 2 or 4 shifted copies of the input window in shared memory
                                    (= floats per shared-memory load); falls back if they do not fit */
-    int32_t reserved[2];        /* must be 0 */
+    int32_t small_templates;    /* templates of <= 128 filters sharing warp tiles (sub-warp segments):
+                                   0 = choose, 1 = on (forces the (8,16) blocking), 2 = off.  Not used with
+                                   SPIIR_PATH_STREAM. */
+    int32_t reserved[1];        /* must be 0 */
 } spiir_options;
 
 /* Build a bank.  All pointers are HOST pointers; the arrays are copied, the caller keeps ownership.
@@ -134,10 +137,12 @@ int spiir_bank_destroy(spiir_bank *bank);
  * stats (nullable, [8] double, HOST) receives {n_slots, n_warp_tiles, n_cta_items, n_rounds,
  * avg_conflict_degree (mean over load phases of the largest number of lanes on one bank group; 1 = conflict
  * free), padding_fraction = 1 - K/n_slots, uniform_groups (1 if every warp position always belongs to the
- * same template shape, which enables per-template barriers), 0}.  Same argument checks as spiir_bank_create. */
+ * same template shape, which enables per-template barriers), segmented (1 if small templates share tiles)}.
+ * pack_small != 0 lays templates of <= 16 * filters_per_thread filters out in shared tiles as spiir_bank_create does
+ * with small_templates = 1.  Same argument checks as spiir_bank_create. */
 int spiir_layout_probe(int32_t n_templates, const int64_t *filter_offsets, const int32_t *delays,
                        int32_t filters_per_thread, int32_t warps_per_cta, int32_t window_copies,
-                       int64_t *slot_of_filter, double *stats);
+                       int64_t *slot_of_filter, double *stats, int32_t pack_small);
 
 /* Introspection. */
 const char *spiir_last_error(void);      /* thread-local message of the last failing call */

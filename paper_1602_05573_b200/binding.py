@@ -29,15 +29,16 @@ class SpiirOptions(ctypes.Structure):
     _fields_ = [("struct_size", ctypes.c_int32), ("path", ctypes.c_int32),
                 ("filters_per_thread", ctypes.c_int32), ("scan_segments", ctypes.c_int32),
                 ("warps_per_cta", ctypes.c_int32), ("window_copies", ctypes.c_int32),
-                ("reserved", ctypes.c_int32 * 2)]
+                ("small_templates", ctypes.c_int32), ("reserved", ctypes.c_int32 * 1)]
 
     def __init__(self, path: int = PATH_AUTO, filters_per_thread: int = 0, scan_segments: int = 0,
-                 warps_per_cta: int = 0, window_copies: int = 0):
+                 warps_per_cta: int = 0, window_copies: int = 0, small_templates: int = 0):
         super().__init__()
         self.struct_size = ctypes.sizeof(SpiirOptions)
         self.path, self.filters_per_thread, self.scan_segments = path, filters_per_thread, scan_segments
         self.warps_per_cta = warps_per_cta
         self.window_copies = window_copies
+        self.small_templates = small_templates
 
 
 def library_path() -> Path:
@@ -83,7 +84,7 @@ def load_library():
     lib.spiir_bank_last_path.argtypes = [vp]
     lib.spiir_version.restype = i32
     lib.spiir_layout_probe.restype = ctypes.c_int
-    lib.spiir_layout_probe.argtypes = [i32, vp, vp, i32, i32, i32, vp, vp]
+    lib.spiir_layout_probe.argtypes = [i32, vp, vp, i32, i32, i32, vp, vp, i32]
     _lib = lib
     return lib
 
@@ -234,7 +235,7 @@ def spiir_version() -> int:
 
 
 def spiir_layout_probe(filter_offsets, delays, filters_per_thread: int = 8, warps_per_cta: int = 16,
-                       window_copies: int = 1):
+                       window_copies: int = 1, pack_small: bool = False):
     """Host-only: the device layout spiir_bank_create would build.  -> (slot_of_filter int64 [K], stats dict)."""
     off = np.ascontiguousarray(filter_offsets, dtype=np.int64)
     d = np.ascontiguousarray(delays, dtype=np.int32)
@@ -243,9 +244,9 @@ def spiir_layout_probe(filter_offsets, delays, filters_per_thread: int = 8, warp
     slots = np.empty(d.size, dtype=np.int64)
     stats = np.zeros(8, dtype=np.float64)
     _check(load_library().spiir_layout_probe(off.size - 1, _ptr(off), _ptr(d), filters_per_thread, warps_per_cta,
-                                             window_copies, _ptr(slots), _ptr(stats)))
+                                             window_copies, _ptr(slots), _ptr(stats), int(pack_small)))
     names = ("n_slots", "n_warp_tiles", "n_cta_items", "n_rounds", "avg_conflict_degree", "padding_fraction",
-             "uniform_groups")
+             "uniform_groups", "segmented")
     return slots, dict(zip(names, stats.tolist()))
 
 

@@ -73,6 +73,7 @@ struct spiir_bank {
     u64* peaks = nullptr;            // [T] packed (power bits << 32 | ~index) of the running call (spiir_filter_peaks)
     float* peak_snr = nullptr;       // internal SNR rows for spiir_filter_peaks without an SNR buffer (multi-round templates)
     int64_t peak_snr_cap = 0;
+    bool segmented = false;          // small templates share warp tiles (SEG kernel variant)
     bool multi_round = false;        // some template spans several CTA rounds (its sums accumulate through the SNR rows)
     WarpWork* work = nullptr;
     int64_t* slot_of_filter = nullptr;
@@ -162,8 +163,19 @@ int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
 // The compiled (F, W) register/warp blockings of the filter kernel: F filters per thread, W warps per CTA.
 // W is chosen so that the register file of an SM is full with one resident CTA (the shared-memory window of
 // a 16 384-sample chunk behind a 16 383-sample history allows only one).
-const void* select_kernel(int F, int W, int NC, bool g, bool peak = false)
+const void* select_kernel(int F, int W, int NC, bool g, bool peak = false, bool seg = false)
 {
+    if (seg) {      // shared tiles of small templates: one blocking, F = 8 / 16 warps (32-filter templates on 4 lanes)
+        if (F != 8 || W != 16) return nullptr;
+#define SPIIR_SEG(P_)                                                                           \
+        if (g) return (const void*)spiir_filter_kernel<8, 16, 1, true, 1, P_, true>;            \
+        if (NC == 4) return (const void*)spiir_filter_kernel<8, 16, 4, false, 1, P_, true>;     \
+        if (NC == 2) return (const void*)spiir_filter_kernel<8, 16, 2, false, 1, P_, true>;     \
+        return (const void*)spiir_filter_kernel<8, 16, 1, false, 1, P_, true>;
+        if (peak) { SPIIR_SEG(true) }
+        SPIIR_SEG(false)
+#undef SPIIR_SEG
+    }
 #define SPIIR_VARIANT_P(F_, W_, M_, P_)                                                        \
         if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true, M_, P_>;               \
         if (NC == 4) return (const void*)spiir_filter_kernel<F_, W_, 4, false, M_, P_>;        \
@@ -181,6 +193,7 @@ const void* select_kernel(int F, int W, int NC, bool g, bool peak = false)
     SPIIR_VARIANT(4, 16, 1)
     SPIIR_VARIANT(4, 32, 1)
     SPIIR_VARIANT(2, 32, 1)
+    SPIIR_VARIANT(1, 32, 1)
 #undef SPIIR_VARIANT
 #undef SPIIR_VARIANT_P
     return nullptr;
@@ -198,8 +211,8 @@ size_t fixed_smem(int F, int W) { return filter_smem_bytes(W, 1, 0, true, nullpt
 // allow the kernel to use all opt-in shared memory (once per variant and bank)
 int configure_kernel(spiir_bank* bk, bool g, const void** fn, bool peak = false)
 {
-    *fn = select_kernel(bk->F, bk->W, bk->NC, g, peak);
-    if (!*fn) return fail(SPIIR_EINVAL, "unsupported blocking F=%d W=%d", bk->F, bk->W);
+    *fn = select_kernel(bk->F, bk->W, bk->NC, g, peak, bk->segmented);
+    if (!*fn) return fail(SPIIR_EINVAL, "unsupported blocking F=%d W=%d%s", bk->F, bk->W, bk->segmented ? " (shared tiles of small templates)" : "");
     if (!bk->configured[g][peak]) {
         CU_TRY(cudaFuncSetAttribute(*fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bk->smem_optin));
         bk->configured[g][peak] = true;
@@ -397,7 +410,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
 
 int choose_F(int32_t T, const int64_t* off, int requested)
 {
-    if (requested == 2 || requested == 4 || requested == 8 || requested == 16) return requested;
+    if (requested == 1 || requested == 2 || requested == 4 || requested == 8 || requested == 16) return requested;
     // Least padded work, weighted by the measured speed of the inner loops on a padding-free bank (cfg3:
     // F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 / 32 warps 44 %, F = 2 / 32 warps 33 % of FP32 peak).
     // F = 2 (64-filter warp tiles) only wins for banks of very small templates (PAPER.md:L335 maps those to one warp).
@@ -422,7 +435,7 @@ int64_t spiir_kernel_launches(void) { return g_launches.load(); }
 int32_t spiir_version(void) { return 100; }
 
 int spiir_layout_probe(int32_t T, const int64_t* off, const int32_t* delays, int32_t F, int32_t W, int32_t NC,
-                       int64_t* slot_of_filter, double* stats)
+                       int64_t* slot_of_filter, double* stats, int32_t pack_small)
 {
     if (!off || !delays) return fail(SPIIR_EINVAL, "null argument");
     if (T <= 0) return fail(SPIIR_EINVAL, "n_templates must be >= 1");
@@ -437,7 +450,7 @@ int spiir_layout_probe(int32_t T, const int64_t* off, const int32_t* delays, int
     HostLayout L;
     try {
         std::vector<float> zeros((size_t)2 * K, 0.f);
-        L = build_layout(T, off, zeros.data(), zeros.data(), delays, F, W, NC);
+        L = build_layout(T, off, zeros.data(), zeros.data(), delays, F, W, NC, pack_small != 0);
     } catch (const std::bad_alloc&) {
         return fail(SPIIR_ENOMEM, "out of host memory building the bank layout");
     }
@@ -450,7 +463,7 @@ int spiir_layout_probe(int32_t T, const int64_t* off, const int32_t* delays, int
         stats[4] = L.avg_conflict_degree;
         stats[5] = L.n_slots ? 1.0 - (double)K / (double)L.n_slots : 0.0;
         stats[6] = L.uniform_groups ? 1.0 : 0.0;
-        stats[7] = 0.0;
+        stats[7] = L.segmented ? 1.0 : 0.0;
     }
     return SPIIR_OK;
 }
@@ -480,14 +493,15 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         if (opt->struct_size < (int32_t)(4 * sizeof(int32_t))) return fail(SPIIR_EINVAL, "bad spiir_options.struct_size");
         memcpy(&o, opt, std::min<size_t>((size_t)opt->struct_size, sizeof(o)));
         if (o.path < SPIIR_PATH_AUTO || o.path > SPIIR_PATH_STREAM) return fail(SPIIR_EINVAL, "bad path option");
-        if (o.filters_per_thread != 0 && o.filters_per_thread != 2 && o.filters_per_thread != 4 &&
-            o.filters_per_thread != 8 && o.filters_per_thread != 16)
-            return fail(SPIIR_EINVAL, "filters_per_thread must be 0, 2, 4, 8 or 16");
+        if (o.filters_per_thread != 0 && o.filters_per_thread != 1 && o.filters_per_thread != 2 &&
+            o.filters_per_thread != 4 && o.filters_per_thread != 8 && o.filters_per_thread != 16)
+            return fail(SPIIR_EINVAL, "filters_per_thread must be 0, 1, 2, 4, 8 or 16");
         if (o.scan_segments < 0) return fail(SPIIR_EINVAL, "scan_segments must be >= 0");
         if (o.warps_per_cta != 0 && o.warps_per_cta != 8 && o.warps_per_cta != 16 && o.warps_per_cta != 32)
             return fail(SPIIR_EINVAL, "warps_per_cta must be 0, 8, 16 or 32");
         if (o.window_copies != 0 && o.window_copies != 1 && o.window_copies != 2 && o.window_copies != 4)
             return fail(SPIIR_EINVAL, "window_copies must be 0, 1, 2 or 4");
+        if (o.small_templates < 0 || o.small_templates > 2) return fail(SPIIR_EINVAL, "small_templates must be 0, 1 or 2");
     }
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0)
@@ -503,6 +517,24 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     const bool stream = (o.path == SPIIR_PATH_STREAM);     // tiny chunks: small CTAs, several per SM
     bk->F = stream && !o.filters_per_thread ? 4 : choose_F(T, off, o.filters_per_thread);
     bk->W = o.warps_per_cta ? o.warps_per_cta : (stream ? 8 : default_warps(bk->F));
+    // Small templates (<= 128 filters) can share warp tiles (PAPER.md:L333-L335 size-aware mapping):
+    // blocking F = 8 / 16 warps.  Taken when asked for, or by itself when it removes >= 25 % of the padded work.
+    if (!stream && o.small_templates != 2 && (o.filters_per_thread == 0 || o.filters_per_thread == 8) &&
+        (o.warps_per_cta == 0 || o.warps_per_cta == 16)) {
+        double plain = 0, packed = 0;
+        bool any_small = false;
+        const int64_t per = 32LL * bk->F;
+        for (int32_t t = 0; t < T; ++t) {
+            const int64_t Kt = off[t + 1] - off[t];
+            plain += (double)((Kt + per - 1) / per * per);
+            const int w = segment_lanes(Kt, 8, true);
+            any_small |= (w < kWarp);
+            packed += w < kWarp ? (double)(w * 8) : (double)((Kt + 255) / 256 * 256);
+        }
+        if (any_small && (o.small_templates == 1 || packed < 0.75 * plain)) {
+            bk->F = 8; bk->W = 16; bk->segmented = true;
+        }
+    }
     if (!valid_blocking(bk->F, bk->W)) {
         const int F = bk->F, W = bk->W;
         free_bank(bk);
@@ -539,7 +571,8 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     }
     HostLayout L;
     try {
-        L = build_layout(T, off, a1, b0, delays, bk->F, bk->W, bk->NC);
+        L = build_layout(T, off, a1, b0, delays, bk->F, bk->W, bk->NC, bk->segmented);
+        bk->segmented = L.segmented;
     } catch (const std::bad_alloc&) {
         free_bank(bk);
         return fail(SPIIR_ENOMEM, "out of host memory building the bank layout");

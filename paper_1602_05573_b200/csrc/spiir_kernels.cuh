@@ -222,6 +222,62 @@ __device__ __forceinline__ void cross_warp_store(const u64* __restrict__ pb, con
     }
 }
 
+// Shared ("segmented") warp tiles: the 32 lanes hold 32/w small templates of w = 4, 8 or 16 lanes each (x F register
+// slots).  Same transpose as warp_reduce_tile; the lane group sums are already per template for w = 8, split in two
+// for w = 4 and joined by one shuffle step for w = 16.  The sums go straight to the templates' SNR rows (8 samples
+// = 64 contiguous bytes per template), no partial buffer and no cross-warp pass.  Every template is summed by the
+// same tree wherever its segment sits in the tile.
+// Largest key among the 8 lanes of a lane group (the 8 samples of one template segment); lane j = 0 commits it.
+__device__ __forceinline__ void seg_peak_commit(u64 key, bool valid, int j, u64* __restrict__ slot)
+{
+    if (!valid) key = 0ull;
+#pragma unroll
+    for (int d = 1; d < 8; d <<= 1) {
+        const u64 o = __shfl_xor_sync(0xffffffffu, key, d);
+        key = o > key ? o : key;
+    }
+    if (j == 0 && key) atomicMax(slot, key);
+}
+
+template <bool PEAK>
+__device__ __forceinline__ void seg_reduce_store(u64 (&S)[kTT], u64* __restrict__ tr, int lane, int w, int n_seg, int nv,
+                                                 u64* __restrict__ out_row0, int64_t ld, u64* __restrict__ peak0 = nullptr,
+                                                 int64_t idx0 = 0)
+{
+    ulonglong2* row = reinterpret_cast<ulonglong2*>(tr + lane * kTrRow);
+#pragma unroll
+    for (int c = 0; c < kTT / 2; ++c) row[c] = make_ulonglong2(S[2 * c], S[2 * c + 1]);
+    __syncwarp();
+    const int g = lane >> 3, j = lane & 7, b = g & 1;
+    const u64* ra = tr + (g * 8 + 4 * b) * kTrRow + j;
+    const u64* rb = tr + (g * 8 + 4 * (1 - b)) * kTrRow + j;
+    const u64 sa = fadd2(fadd2(ra[0], ra[kTrRow]), fadd2(ra[2 * kTrRow], ra[3 * kTrRow]));   // lanes g*8 + 4b .. +3
+    const u64 sb = fadd2(fadd2(rb[0], rb[kTrRow]), fadd2(rb[2 * kTrRow], rb[3 * kTrRow]));   // the other half of the group
+    __syncwarp();
+    if (w == 4) {
+        const int seg_a = 2 * g + b, seg_b = 2 * g + 1 - b;
+        const bool va = j < nv && seg_a < n_seg, vb = j < nv && seg_b < n_seg;
+        if (out_row0) {
+            if (va) out_row0[(int64_t)seg_a * ld + j] = sa;
+            if (vb) out_row0[(int64_t)seg_b * ld + j] = sb;
+        }
+        if (PEAK && peak0) {
+            seg_peak_commit(peak_key(sa, idx0 + j), va, j, peak0 + seg_a);
+            seg_peak_commit(peak_key(sb, idx0 + j), vb, j, peak0 + seg_b);
+        }
+    } else {
+        u64 P = fadd2(sa, sb);                                         // 8 lanes
+        int seg = g;
+        if (w == 16) {
+            P = fadd2(P, __shfl_xor_sync(0xffffffffu, P, 8));
+            seg = g >> 1;
+        }
+        const bool v = j < nv && seg < n_seg && (w == 8 || b == 0);
+        if (out_row0 && v) out_row0[(int64_t)seg * ld + j] = P;
+        if (PEAK && peak0) seg_peak_commit(peak_key(P, idx0 + j), v, j, peak0 + seg);
+    }
+}
+
 // Shared memory of the filter kernel, in this order:
 //   NC window copies of `cstride` floats each (absent when GMEM_X), W transpose scratches, kPB x W x kTS partial sums,
 //   W x kPB mbarriers
@@ -239,7 +295,8 @@ __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_l
 // MINB = CTAs the register allocation must leave room for on one SM (tiny-chunk streaming: several small CTAs
 // per SM overlap one CTA's coefficient loads with another's arithmetic).
 // PEAK compiles the fused trigger reduction in (spiir_filter_peaks); the plain kernel is untouched by it.
-template <int F, int W, int NC, bool GMEM_X, int MINB = 1, bool PEAK = false>
+// SEG compiles the shared-tile path for banks of small templates in.
+template <int F, int W, int NC, bool GMEM_X, int MINB = 1, bool PEAK = false, bool SEG = false>
 __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const FilterParams p)
 {
     static_assert(!GMEM_X || NC == 1, "the global-memory window variant reads scalars");
@@ -299,8 +356,10 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
         const int r0 = p.item_round0[item], r1 = p.item_round0[item + 1];
         for (int r = r0; r < r1; ++r) {
-            const WarpWork ww = p.work[r * W + warp];
+            WarpWork ww = p.work[r * W + warp];
             const bool active = ww.tile >= 0;
+            int seg_w = 0, seg_n = 0;                  // > 0: this warp's tile is shared by seg_n templates of seg_w lanes
+            if (SEG) { seg_w = (ww.first >> 8) & 0xff; seg_n = ww.first >> 16; ww.first &= 0xff; }
             float ar[F];
             u64 AI[F], B[F], Y[F];
             int xo[F];
@@ -370,14 +429,19 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                             if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
                             else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
                             if (sums) {
-                                const u64 P = warp_reduce_tile(S, mytr, lane);
-                                if (lane < kTT) mypart[tt + lane] = P;
+                                if (SEG && seg_w) {
+                                    seg_reduce_store<PEAK>(S, mytr, lane, seg_w, seg_n, nv, (!PEAK || out_row) ? out_row + st + tt : nullptr, p.ld,
+                                                           peak, idx_row + st + tt);
+                                } else {
+                                    const u64 P = warp_reduce_tile(S, mytr, lane);
+                                    if (lane < kTT) mypart[tt + lane] = P;
+                                }
                             }
                         }
                     }
                     if (sums) {
                         __syncthreads();
-                        if (active)
+                        if (active && !(SEG && seg_w))
                             cross_warp_store<TS, PEAK>(part64 + (size_t)buf * W * TS, ww, warp, lane, ns, (!PEAK || out_row) ? out_row + st : nullptr, accumulate, peak, idx_row + st);
                     }
                 }

@@ -43,6 +43,7 @@ struct HostLayout {
     // work list: items (one CTA at a time), each with >= 1 rounds of W warp entries
     std::vector<int32_t> item_round0;   // [n_items+1] first round of each item
     std::vector<WarpWork> work;         // [n_rounds * W]
+    bool segmented = false;             // some warp tiles hold several small templates (tile_begin is then not a CSR)
     std::vector<int32_t> canon;         // [2W] (first, count) of every warp position when uniform_groups, else (-1, 0)
     bool uniform_groups = true;         // every warp position has the same (first, count) in all rounds it is active in
     double avg_conflict_degree = 0.0;   // mean over load phases of the max key multiplicity (diagnostic)
@@ -121,8 +122,19 @@ inline void deal_groups(const int32_t* d, const std::vector<int64_t>& order, int
     }
 }
 
+// Lanes a small template occupies in a shared ("segmented") warp tile: the smallest of 4, 8, 16 whose lanes x F
+// register slots hold its K_t filters; 32 = a template that gets warp tiles of its own (PAPER.md:L333-L335 maps
+// templates of <= 32 filters to one warp; here several of them share one warp so that every lane still runs F filters).
+inline int segment_lanes(int64_t Kt, int F, bool pack_small)
+{
+    if (!pack_small) return kWarp;
+    for (int w : {4, 8, 16})
+        if ((int64_t)w * F >= Kt) return w;
+    return kWarp;
+}
+
 inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, const float* b0,
-                               const int32_t* d, int F, int W, int NC = 1)
+                               const int32_t* d, int F, int W, int NC = 1, bool pack_small = false)
 {
     HostLayout L;
     L.F = F;
@@ -132,9 +144,35 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
     L.tile_begin.resize((size_t)T + 1);
     int64_t tiles = 0;
     const int64_t per_tile = (int64_t)kWarp * F;
-    for (int32_t t = 0; t < T; ++t) {
-        L.tile_begin[t] = tiles;
-        tiles += (off[t + 1] - off[t] + per_tile - 1) / per_tile;
+    // tile of every template; small templates of one size class that follow each other share a tile
+    std::vector<int> seg_w((size_t)T, kWarp), seg_idx((size_t)T, 0);
+    std::vector<int> tile_nseg;                       // templates in a tile (0 for regular tiles)
+    {
+        int open_w = 0, open_used = 0;
+        int64_t open_tile = -1;
+        for (int32_t t = 0; t < T; ++t) {
+            const int64_t Kt = off[t + 1] - off[t];
+            const int w = segment_lanes(Kt, F, pack_small);
+            seg_w[t] = w;
+            if (w == kWarp) {
+                open_w = 0;
+                L.tile_begin[t] = tiles;
+                const int64_t nt = (Kt + per_tile - 1) / per_tile;
+                tiles += nt;
+                tile_nseg.resize((size_t)tiles, 0);
+            } else {
+                if (open_w != w || open_used == kWarp / w) {
+                    open_tile = tiles++;
+                    tile_nseg.resize((size_t)tiles, 0);
+                    open_w = w;
+                    open_used = 0;
+                }
+                L.tile_begin[t] = open_tile;
+                seg_idx[t] = open_used++;
+                tile_nseg[(size_t)open_tile] = open_used;
+                L.segmented = true;
+            }
+        }
     }
     L.tile_begin[T] = tiles;
     L.n_tiles = tiles;
@@ -154,7 +192,28 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
         order.resize((size_t)Kt);
         std::iota(order.begin(), order.end(), k0);
         std::stable_sort(order.begin(), order.end(), [&](int64_t x, int64_t y) { return d[x] < d[y]; });
-        const int64_t nt = L.tile_begin[t + 1] - L.tile_begin[t];
+        if (seg_w[t] < kWarp) {
+            // small template: lanes [seg * w, seg * w + w) of a shared tile, filter i (delay order) -> lane i % w, slot i / w
+            const int w = seg_w[t];
+            const int64_t tile = L.tile_begin[t];
+            for (int64_t i = 0; i < (int64_t)w * F; ++i) {
+                const int64_t s = (tile * F + i / w) * kWarp + (int64_t)seg_idx[t] * w + i % w;
+                if (i < Kt) {
+                    const int64_t k = order[(size_t)i];
+                    L.ar[s] = a1[2 * k];
+                    L.ai2[2 * s] = -a1[2 * k + 1];
+                    L.ai2[2 * s + 1] = a1[2 * k + 1];
+                    L.b[2 * s] = b0[2 * k];
+                    L.b[2 * s + 1] = b0[2 * k + 1];
+                    L.dly[s] = d[k];
+                    L.slot_of_filter[k] = s;
+                } else {
+                    L.dly[s] = d[order[0]];           // null filter: any valid window position
+                }
+            }
+            continue;
+        }
+        const int64_t nt = (Kt + per_tile - 1) / per_tile;
         const int G = (int)(nt * F);
         deal_groups(d, order, G, NC, groups, degree_sum, n_phases);
         for (int g = 0; g < G; ++g) {
@@ -181,6 +240,24 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
             if (groups[g].empty())
                 for (int l = 0; l < kWarp; ++l) L.dly[(L.tile_begin[t] * F + g) * kWarp + l] = d[order[0]];
     }
+    if (L.segmented) {
+        // conflict statistics of the shared tiles (their lanes are not dealt: neighbours' delays are independent)
+        std::vector<char> real((size_t)L.n_slots, 0);
+        for (int64_t k = 0; k < K; ++k) real[(size_t)L.slot_of_filter[k]] = 1;
+        const int P = kWarp / NC;
+        std::vector<int> cnt(P);
+        for (int64_t tile = 0; tile < tiles; ++tile) {
+            if (!tile_nseg[(size_t)tile]) continue;
+            for (int g = 0; g < F * NC; ++g) {
+                const int64_t s0 = (tile * F + g / NC) * kWarp + (int64_t)(g % NC) * P;
+                std::fill(cnt.begin(), cnt.end(), 0);
+                int mx = 0;
+                for (int l = 0; l < P; ++l)
+                    if (real[(size_t)(s0 + l)]) mx = std::max(mx, ++cnt[conflict_key(L.dly[(size_t)(s0 + l)], NC, P)]);
+                if (mx) { degree_sum += mx; ++n_phases; }
+            }
+        }
+    }
     L.avg_conflict_degree = n_phases ? degree_sum / (double)n_phases : 0.0;
 
     // Work list.  Templates with <= W tiles share an item round with their neighbours (greedy, in bank
@@ -195,7 +272,15 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
         cur.clear();
     };
     for (int32_t t = 0; t < T; ++t) {
-        const int64_t nt = L.tile_begin[t + 1] - L.tile_begin[t];
+        if (seg_w[t] < kWarp) {
+            // a shared tile is one warp's work; `first` also carries the segment width and the number of templates
+            if (seg_idx[t] != 0) continue;
+            if ((int)cur.size() + 1 > W) flush();
+            const int first = (int)cur.size();
+            cur.push_back(WarpWork{(int32_t)L.tile_begin[t], t, first | (seg_w[t] << 8) | (tile_nseg[(size_t)L.tile_begin[t]] << 16), 1});
+            continue;
+        }
+        const int64_t nt = (off[t + 1] - off[t] + per_tile - 1) / per_tile;
         if (nt <= W) {
             if ((int64_t)cur.size() + nt > W) flush();
             const int first = (int)cur.size();
@@ -217,10 +302,12 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
     // otherwise a fast warp could enter a hardware barrier that a slower group of another shape still uses.
     {
         std::vector<int32_t> first(W, -1), count(W, -1);
+        if (L.segmented) L.uniform_groups = false;      // shared tiles store their sums themselves, behind CTA-wide barriers
         for (size_t i = 0; i < L.work.size(); ++i) {
             const WarpWork& w = L.work[i];
             if (w.tile < 0) continue;
             const int pos = (int)(i % (size_t)W);
+            if (!L.uniform_groups) break;
             if (first[pos] < 0) { first[pos] = w.first; count[pos] = w.count; }
             else if (first[pos] != w.first || count[pos] != w.count) { L.uniform_groups = false; break; }
         }

@@ -27,13 +27,13 @@ def env():
     return pkg, oracle, torch
 
 
-def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=False):
+def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=False, small=0):
     """Filter inp.x through a fresh bank in the given chunking; returns complex64 [T or len(rows), N]."""
     pkg, _, torch = env
     N = inp.n_samples
     chunks = [N] if chunks is None else list(chunks)
     assert sum(chunks) == N
-    opt = pkg.SpiirOptions(path=path, filters_per_thread=F, scan_segments=segments)
+    opt = pkg.SpiirOptions(path=path, filters_per_thread=F, scan_segments=segments, small_templates=small)
     with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank:
         if host:
             out = np.empty((inp.n_templates, N), dtype=np.complex64)
@@ -149,6 +149,26 @@ def test_bank_of_very_small_templates(env):
     ref = env[1].run_inputs(inp.select_templates(rows))
     check(run_gpu(env, inp, chunks=[400, 500], rows=rows), ref)
     check(run_gpu(env, inp, chunks=[64] * 14 + [4], path=3, rows=rows), ref)
+
+
+def test_small_templates_share_warp_tiles(env):
+    # sub-warp segments: 4-, 8- and 16-lane segments, partially filled tiles, size
+    # classes changing along the bank, and large templates in between
+    counts = [32, 17, 8, 1, 32, 30, 2, 25, 64, 33, 60, 128, 100, 65, 700, 12, 12, 12, 128, 129, 5] * 6
+    inp = spiir_inputs.make_random_bank(62, counts, 1100, d_max=400)
+    ref = env[1].run_inputs(inp)
+    for path in (1, 2):
+        check(run_gpu(env, inp, chunks=[500, 7, 593], path=path, small=1), ref)
+    a = run_gpu(env, inp, chunks=[500, 600], path=1, small=1)
+    assert np.array_equal(a.view(np.float32), run_gpu(env, inp, chunks=[500, 600], path=1, small=1).view(np.float32))
+    # a template's sums do not depend on which segment of which tile it landed in
+    perm = np.random.default_rng(1).permutation(len(counts))
+    b = run_gpu(env, inp.select_templates(perm), chunks=[500, 600], path=1, small=1)
+    assert np.array_equal(b.view(np.float32), a[perm].view(np.float32))
+    # chosen by itself for a bank of tiny templates, and the host entry works on it
+    tiny = spiir_inputs.make_random_bank(63, [32, 20, 31] * 100, 600, d_max=300)
+    check(run_gpu(env, tiny, chunks=[600]), env[1].run_inputs(tiny))
+    check(run_gpu(env, tiny, chunks=[300, 300], host=True), env[1].run_inputs(tiny))
 
 
 def test_zero_delay_and_constant_delay(env):
@@ -368,6 +388,15 @@ def test_filter_peaks_against_oracle(env, path, with_snr):
     chunks = chunks[:] if sum(chunks) <= inp.n_samples else chunks
     assert sum(chunks) <= inp.n_samples
     check_peaks(pkg, torch, oracle, inp, chunks, pkg.SpiirOptions(path=path), with_snr, ref)
+
+
+def test_filter_peaks_on_shared_tiles(env):
+    pkg, oracle, torch = env
+    counts = [32, 17, 8, 1, 32, 30, 2, 25, 64, 33, 60, 128, 100, 65, 700, 12] * 3
+    inp = spiir_inputs.make_random_bank(64, counts, 1500, d_max=300)
+    ref = oracle.run_inputs(inp)
+    for with_snr in (False, True):
+        check_peaks(pkg, torch, oracle, inp, [700, 9, 791], pkg.SpiirOptions(path=1, small_templates=1), with_snr, ref)
 
 
 def test_filter_peaks_cfg3_blocking_and_exact_tie(env):

@@ -88,6 +88,31 @@ def test_work_list_counts(pkg):
     assert st["n_warp_tiles"] == 40 and st["n_cta_items"] == 1 and st["n_rounds"] == 3
 
 
+def test_small_templates_pack_into_shared_tiles(pkg):
+    counts = [32, 17, 8, 1, 32, 30, 2, 25, 64, 33, 700, 12, 128, 129]
+    inp = spiir_inputs.make_random_bank(9, counts, 8, d_max=300)
+    plain, st0 = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, 2, False)
+    slots, st = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, 2, True)
+    assert st0["segmented"] == 0 and st["segmented"] == 1 and st["uniform_groups"] == 0
+    assert st["n_slots"] <= 0.5 * st0["n_slots"]
+    assert len(set(slots.tolist())) == slots.size
+    F = 8
+    tile = slots // (32 * F)
+    lane = slots % 32
+    for t, k in enumerate(counts):
+        s = slice(inp.offsets[t], inp.offsets[t + 1])
+        if k <= 16 * F:
+            w = next(w for w in (4, 8, 16) if w * F >= k)
+            assert len(set(tile[s].tolist())) == 1                      # one tile
+            lo = lane[s].min() // w * w
+            assert lane[s].min() >= lo and lane[s].max() < lo + w        # inside one aligned segment of w lanes
+        else:
+            assert len(set(tile[s].tolist())) == -(-k // (32 * F))
+    # 32 and 17 filters (4 lanes) share a tile; the class change to 8 filters (4 lanes too) keeps sharing; 64 -> 8 lanes opens a new one
+    assert tile[inp.offsets[0]] == tile[inp.offsets[1]] == tile[inp.offsets[2]]
+    assert tile[inp.offsets[8]] != tile[inp.offsets[7]]
+
+
 def test_probe_validates_arguments(pkg):
     with pytest.raises(pkg.SpiirError):
         pkg.spiir_layout_probe(np.array([0, 2]), np.array([0, -1], np.int32))
