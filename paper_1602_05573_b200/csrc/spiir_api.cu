@@ -408,22 +408,26 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     return SPIIR_OK;
 }
 
-int choose_F(int32_t T, const int64_t* off, int requested)
+// Relative cost per padded filter slot of the compiled blockings, measured on padding-free banks (cfg3 for F >= 8,
+// banks of 32- to 128-filter templates below): F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 ~ 42 %,
+// F = 2 ~ 29 %, F = 1 (one warp per template) ~ 21 % of FP32 peak; shared tiles (F = 8) ~ 34.5 %.
+double slot_cost(int F) { return F == 16 ? 1.0 : (F == 8 ? 1.05 : (F == 4 ? 1.3 : (F == 2 ? 1.85 : 2.6))); }
+constexpr double kSharedTileCost = 1.57;
+
+int choose_F(int32_t T, const int64_t* off, int requested, double* cost_out = nullptr)
 {
-    if (requested == 1 || requested == 2 || requested == 4 || requested == 8 || requested == 16) return requested;
-    // Least padded work, weighted by the measured speed of the inner loops on a padding-free bank (cfg3:
-    // F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 / 32 warps 44 %, F = 2 / 32 warps 33 % of FP32 peak).
-    // F = 2 (64-filter warp tiles) only wins for banks of very small templates (PAPER.md:L335 maps those to one warp).
     double best = 0;
     int bestF = 0;
-    for (int F : {16, 8, 4, 2}) {
+    for (int F : {16, 8, 4, 2, 1}) {
+        if (requested && F != requested) continue;
         const int64_t per = 32LL * F;
         double padded = 0;
         for (int32_t t = 0; t < T; ++t) padded += (double)((off[t + 1] - off[t] + per - 1) / per * per);
-        padded *= (F == 16 ? 1.0 : (F == 8 ? 1.05 : (F == 4 ? 1.22 : 1.63)));
+        padded *= slot_cost(F);
         if (!bestF || padded < best) { best = padded; bestF = F; }
     }
-    return bestF;
+    if (cost_out) *cost_out = best;
+    return bestF ? bestF : 8;
 }
 
 }  // namespace
@@ -515,30 +519,24 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->opt = o;
     bk->T = T; bk->K = K; bk->D = D;
     const bool stream = (o.path == SPIIR_PATH_STREAM);     // tiny chunks: small CTAs, several per SM
-    bk->F = stream && !o.filters_per_thread ? 4 : choose_F(T, off, o.filters_per_thread);
+    double plain_cost = 0;
+    bk->F = stream && !o.filters_per_thread ? 4 : choose_F(T, off, o.filters_per_thread, &plain_cost);
     bk->W = o.warps_per_cta ? o.warps_per_cta : (stream ? 8 : default_warps(bk->F));
     // Small templates (<= 128 filters) can share warp tiles (PAPER.md:L333-L335 size-aware mapping):
-    // blocking F = 8 / 16 warps.  Taken when asked for, or by itself when it removes >= 25 % of the padded work.
+    // blocking F = 8 / 16 warps.  Taken when asked for, or by itself when its estimated cost is lower.
     if (!stream && o.small_templates != 2 && (o.filters_per_thread == 0 || o.filters_per_thread == 8) &&
         (o.warps_per_cta == 0 || o.warps_per_cta == 16)) {
-        double plain = 0, packed = 0;
+        double packed = 0;
         bool any_small = false;
-        const int64_t per = 32LL * bk->F;
         for (int32_t t = 0; t < T; ++t) {
             const int64_t Kt = off[t + 1] - off[t];
-            plain += (double)((Kt + per - 1) / per * per);
             const int w = segment_lanes(Kt, 8, true);
             any_small |= (w < kWarp);
-            packed += w < kWarp ? (double)(w * 8) : (double)((Kt + 255) / 256 * 256);
+            packed += w < kWarp ? kSharedTileCost * (double)(w * 8) : slot_cost(8) * (double)((Kt + 255) / 256 * 256);
         }
-        if (any_small && (o.small_templates == 1 || packed < 0.75 * plain)) {
+        if (any_small && (o.small_templates == 1 || packed < plain_cost)) {
             bk->F = 8; bk->W = 16; bk->segmented = true;
         }
-    }
-    if (!valid_blocking(bk->F, bk->W)) {
-        const int F = bk->F, W = bk->W;
-        free_bank(bk);
-        return fail(SPIIR_EINVAL, "unsupported blocking: filters_per_thread %d with warps_per_cta %d", F, W);
     }
     cudaDeviceProp prop;
     cudaError_t e = cudaGetDeviceProperties(&prop, device);
