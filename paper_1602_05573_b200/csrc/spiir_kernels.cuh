@@ -11,10 +11,19 @@
 //     t  = (-a_im, a_im) * (y_im, y_re) + t
 //     y' = (a_re, a_re) * (y_re, y_im) + t
 //     S += y'
-// = 4 issue slots per filter-sample instead of 8 scalar ones.  Per-thread partial sums of TT = 8
-// consecutive samples are reduced across the warp with a transposing shuffle butterfly (fixed order, no
-// atomics -> bitwise reproducible), staged in shared memory per 64-sample super tile, summed across the
-// warps of a template and written with coalesced 8-byte stores.
+// = 4 packed instructions per filter-sample instead of 8 scalar ones (the register file, not the pipe, then bounds
+// the rate: fp32_pipe_probe.cu).  Per-thread partial sums of TT = 8 consecutive samples are
+// reduced across the warp through a per-warp shared-memory transpose (fixed order, no atomics -> bitwise
+// reproducible), collected per super tile in shared memory, handed over between the warps of a template with
+// mbarriers, summed in warp order and written with coalesced 8-byte stores.
+//
+// Kernels in this file:
+//   spiir_filter_kernel<F, W, NC, GMEM_X, MINB, PEAK, SEG>  the blocked kernel (throughput path, both passes of the
+//       time-parallel scan path, long calls of streaming banks); PEAK adds the fused trigger reduction, SEG the shared
+//       warp tiles of small templates
+//   spiir_stream_kernel<F, NC> + spiir_stream_combine_kernel   tiny chunks: independent warps + ordered combine
+//   spiir_scan_carry_kernel                                    carry combine of the scan path, in double
+//   spiir_unpack_peaks_kernel, spiir_permute_state_kernel      small utilities
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

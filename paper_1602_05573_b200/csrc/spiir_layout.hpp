@@ -2,12 +2,14 @@
 // "parameter array ... aligned and continuous ... coalesed memory access").
 //
 // A template's filters are sorted by delay, then dealt to "groups" of 32 (one filter per lane of a
-// warp for one register slot f).  All 32 lanes of a group read x[n - d] from shared memory in the same
-// instruction, so the group is conflict-free iff its delays are distinct modulo 32 (or equal).  The
-// dealing first builds as many perfect groups as the residue histogram allows and spreads the rest
-// evenly, which keeps the average conflict degree near 1.4 for uniformly random delays (3.4 undealt).
+// warp for one register slot f).  All 32 lanes of a group read their delayed input from shared memory in the same
+// instruction, NC floats each, served in NC phases of 32/NC lanes; a phase is conflict-free iff the lanes' keys
+// ceil(d / NC) mod (32 / NC) are distinct (or the delays equal).  The dealing first builds as many perfect phases as
+// the key histogram allows and spreads the rest evenly, which keeps the average conflict degree near 1.4 / 1.2 / 1.1
+// for NC = 1 / 2 / 4 and uniformly random delays (3.4 undealt, NC = 1).
 // F consecutive groups form a warp tile (32 lanes x F register slots); tiles are padded with null
-// filters (a1 = b0 = 0) whose delay copies a real filter of the same group (same address = broadcast).
+// filters (a1 = b0 = 0) whose delay copies a real filter of the same phase (same address = broadcast).
+// Templates of <= 16 F filters can instead share a tile in aligned segments of 4, 8 or 16 lanes (pack_small).
 //
 // The layout of a template is a pure function of that template's own (a1, b0, d) arrays, so results are
 // bitwise independent of the template's position in the bank (invariants).
