@@ -161,6 +161,15 @@ def run_ours(args):
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if not pkg.library_path().exists():
+        # the in-tree library normally travels with the repo; build it once (local rank 0) if it does not
+        if local_rank == 0:
+            from paper_1602_05573_b200.build import build as build_cuda
+            build_cuda()
+        else:
+            t_wait = time.time()
+            while not pkg.library_path().exists() and time.time() - t_wait < 600:
+                time.sleep(1.0)
     pkg.load_library()
 
     # every rank filters its own seeded bank of the config's size (weak scaling, no exchange step)

@@ -23,6 +23,9 @@ def env():
         pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
     import oracle
     import paper_1602_05573_b200 as pkg
+    if not pkg.library_path().exists():
+        import __graft_entry__ as entry
+        entry.build()
     pkg.load_library()
     return pkg, oracle, torch
 
