@@ -298,8 +298,22 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
     void* args[] = {(void*)&p};
     CU_TRY(cudaLaunchKernel(fn, dim3((unsigned)ctas, 1, 1), dim3(kWarp * kStreamWarps, 1, 1), args, smem, st));
     const int64_t total = bk->T * n;
-    spiir_stream_combine_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(bk->stream_scratch, bk->tile_begin,
-                                                                             (int32_t)bk->T, (int32_t)n, snr, ld, peaks);
+    {
+        // programmatic dependent launch: the combine grid is set up while the streaming kernel drains and waits
+        // (griddepcontrol.wait in the kernel) for its results
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)((total + 255) / 256), 1, 1);
+        cfg.blockDim = dim3(256, 1, 1);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        CU_TRY(cudaLaunchKernelEx(&cfg, spiir_stream_combine_kernel, (const u64*)bk->stream_scratch,
+                                  (const int64_t*)bk->tile_begin, (int32_t)bk->T, (int32_t)n, snr, ld, peaks));
+    }
     g_launches.fetch_add(2, std::memory_order_relaxed);
     CU_TRY(cudaGetLastError());
     bk->last_path = SPIIR_PATH_STREAM;

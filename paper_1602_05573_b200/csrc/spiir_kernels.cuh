@@ -583,6 +583,7 @@ __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, con
     if (i >= (int64_t)n_templates * n) return;
     const int32_t t = (int32_t)(i / n), j = (int32_t)(i % n);
     const int64_t t0 = tile_begin[t], t1 = tile_begin[t + 1];
+    asm volatile("griddepcontrol.wait;" ::: "memory");     // launched early (PDL): the streaming kernel's rows from here on
     u64 acc = scratch[t0 * kStreamMax + j];
     // loads 16 tiles ahead of the (ordered) additions: the chain of adds is short, the chain of L2 latencies is not
     for (int64_t tile = t0 + 1; tile < t1; tile += 16) {
