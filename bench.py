@@ -158,9 +158,18 @@ def run_ours(args):
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the SPIIR library has no CPU fallback")
-    torch.cuda.set_device(local_rank)
+    n_dev = torch.cuda.device_count()
+    # fewer GPUs than ranks (or SPIIR_BENCH_BACKEND=gloo): a functional check of the multi-rank path only -- NCCL cannot put
+    # two ranks on one GPU, so the timing exchange then goes over gloo on the host
+    oversubscribed = world > 1 and (local_rank >= n_dev or os.environ.get("SPIIR_BENCH_BACKEND") == "gloo")
+    dev_index = local_rank % n_dev
+    torch.cuda.set_device(dev_index)
+    red_dev = "cpu" if oversubscribed else "cuda"
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if oversubscribed:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", dev_index))
     if not pkg.library_path().exists():
         # the in-tree library normally travels with the repo; build it once (local rank 0) if it does not
         if local_rank == 0:
@@ -183,7 +192,7 @@ def run_ours(args):
         args.path = pkg.PATH_STREAM            # tiny chunks over a large bank: the HBM-bound streaming blocking
     opt = pkg.SpiirOptions(path=args.path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta,
                            window_copies=args.window_copies, scan_segments=args.scan_segments)
-    bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, local_rank, opt)
+    bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, dev_index, opt)
     x = torch.from_numpy(inp.x).cuda()
     keep_whole = (T * N * 8) <= args.max_snr_bytes
     snr = torch.empty((T, N if keep_whole else L), dtype=torch.complex64, device="cuda")
@@ -218,7 +227,7 @@ def run_ours(args):
     launches0 = pkg.spiir_kernel_launches()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(n_calls + 1)] for _ in range(args.steps)]
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clocks:
+    with ClockSampler(dev_index) as clocks:
         barrier()
         start.record(stream)
         for s in range(args.steps):
@@ -228,7 +237,7 @@ def run_ours(args):
     launches = pkg.spiir_kernel_launches() - launches0
     elapsed_ms = start.elapsed_time(stop)
     call_ms = [ev[s][i].elapsed_time(ev[s][i + 1]) for s in range(args.steps) for i in range(n_calls)]
-    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=red_dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     elapsed_ms_max = float(t.item())
@@ -304,7 +313,7 @@ def run_ours(args):
             e2e_step()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        tt = torch.tensor([dt], dtype=torch.float64, device=red_dev)
         if world > 1:
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         line["e2e"] = {"value": world * fs_step * e2e_steps / float(tt.item()), "unit": UNIT,

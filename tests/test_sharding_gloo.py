@@ -34,6 +34,7 @@ def test_shard_templates_balances_and_partitions():
 
 def _worker(rank, world, port, q):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    os.environ.setdefault("GLOO_SOCKET_IFNAME", "lo")      # the container hostname may not resolve
     import torch
     import torch.distributed as dist
     import oracle
