@@ -40,8 +40,10 @@ FLOPS_PER_FILTER_SAMPLE = 12          # complex*complex 6 + real*complex 2 + com
 N_SM, LANES, BOOST_HZ = 148, 128, 1.965e9   # B200: SMs x FP32 lanes x 2 flops x clocks.max.sm (MEASURED_PEAKS.json sm_max_mhz)
 FP32_PEAK_TFLOPS = N_SM * LANES * 2 * BOOST_HZ / 1e12    # 74.4 TFLOP/s, derivation in DESIGN.md section 7
 # dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch (cfg3, default blocking, 8192 samples)
-# from the committed ncu --set full capture profiles/r01c_filter_kernel_full.md: 135.8 MB + 245.7 MB
-NCU_TRAFFIC_CFG3_LAUNCH = 381.6e6
+# from the committed ncu --set full capture profiles/r01c_filter_kernel_full.md: 135.8 MB + 246.2 MB
+NCU_TRAFFIC_CFG3_LAUNCH = 382.0e6
+# the same for one spiir_stream_kernel launch of cfg4 (16 samples), profiles/r01c_cfg4_stream_launches.md: 165.2 MB + 22.2 MB
+NCU_TRAFFIC_CFG4_LAUNCH = 187.4e6
 
 
 def measured_hbm_peak():
@@ -254,6 +256,8 @@ def run_ours(args):
     default_blocking = not (args.filters_per_thread or args.warps_per_cta or args.window_copies or args.path)
     if traffic is None and args.config == 3 and default_blocking:
         traffic = NCU_TRAFFIC_CFG3_LAUNCH
+    if traffic is None and args.config == 4 and not (args.filters_per_thread or args.warps_per_cta or args.window_copies):
+        traffic = NCU_TRAFFIC_CFG4_LAUNCH
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved_tflops / FP32_PEAK_TFLOPS, "traffic": traffic,
                 "kernel": "spiir_filter_kernel", "launch_ms": avg_call_s * 1e3 / launches_per_call,
@@ -274,8 +278,8 @@ def run_ours(args):
         bytes_call = inp.n_filters * 40.0 + 8.0 * T * L + 4.0 * L     # 24 B coefficients + 8 B state in + 8 B state out per filter
         peak_gbs, peak_src = measured_hbm_peak()
         roofline = {"bound": "hbm", "achieved": bytes_call / avg_call_s / 1e9, "peak": peak_gbs, "unit": "GB/s",
-                    "frac": bytes_call / avg_call_s / 1e9 / peak_gbs, "traffic": args.ncu_traffic_bytes,
-                    "kernel": "spiir_filter_kernel", "launch_ms": avg_call_s * 1e3 / launches_per_call,
+                    "frac": bytes_call / avg_call_s / 1e9 / peak_gbs, "traffic": traffic,
+                    "kernel": "spiir_stream_kernel (+ spiir_stream_combine_kernel)", "launch_ms": avg_call_s * 1e3 / launches_per_call,
                     "launches_per_call": launches_per_call, "call_ms": avg_call_s * 1e3, "peak_source": peak_src,
                     "algorithmic_bytes_per_call": bytes_call}
 
