@@ -42,8 +42,8 @@ FP32_PEAK_TFLOPS = N_SM * LANES * 2 * BOOST_HZ / 1e12    # 74.4 TFLOP/s, derivat
 # dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch (cfg3, default blocking, 8192 samples)
 # from the committed ncu --set full capture profiles/r01c_filter_kernel_full.md: 135.8 MB + 246.2 MB
 NCU_TRAFFIC_CFG3_LAUNCH = 382.0e6
-# the same for one spiir_stream_kernel launch of cfg4 (16 samples), profiles/r01c_cfg4_stream_launches.md: 165.2 MB + 22.2 MB
-NCU_TRAFFIC_CFG4_LAUNCH = 187.4e6
+# the same for one spiir_stream_kernel launch of cfg4 (16 samples), profiles/r01c_cfg4_stream_launches.md: 144.7 MB + 18.8 MB
+NCU_TRAFFIC_CFG4_LAUNCH = 163.5e6
 
 
 def measured_hbm_peak():
@@ -275,7 +275,7 @@ def run_ours(args):
                "real_time_us_per_call": 1e6 * L / spiir_inputs.FS}
     if L <= 64:
         # tiny chunks: every call streams the whole bank through the SMs once -> HBM roofline
-        bytes_call = inp.n_filters * 40.0 + 8.0 * T * L + 4.0 * L     # 24 B coefficients + 8 B state in + 8 B state out per filter
+        bytes_call = inp.n_filters * 36.0 + 8.0 * T * L + 4.0 * L     # 20 B coefficients + 8 B state in + 8 B state out per filter
         peak_gbs, peak_src = measured_hbm_peak()
         roofline = {"bound": "hbm", "achieved": bytes_call / avg_call_s / 1e9, "peak": peak_gbs, "unit": "GB/s",
                     "frac": bytes_call / avg_call_s / 1e9 / peak_gbs, "traffic": traffic,

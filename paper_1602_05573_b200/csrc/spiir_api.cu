@@ -63,7 +63,7 @@ struct spiir_bank {
     double avg_conflict_degree = 0.0;
     spiir_options opt{};
     // device bank
-    float *ar = nullptr, *ai2 = nullptr, *b = nullptr, *y = nullptr;
+    float *ar = nullptr, *ai = nullptr, *b = nullptr, *y = nullptr;
     int32_t* dly = nullptr;
     int32_t* item_round0 = nullptr;
     int32_t* canon = nullptr;
@@ -111,7 +111,7 @@ int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 void free_bank(spiir_bank* bk)
 {
     if (!bk) return;
-    cudaFree(bk->ar); cudaFree(bk->ai2); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
+    cudaFree(bk->ar); cudaFree(bk->ai); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
     cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->tile_begin); cudaFree(bk->stream_scratch); cudaFree(bk->peaks); cudaFree(bk->peak_snr); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
     cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
     cudaFree(bk->hx); cudaFree(bk->hsnr[0]); cudaFree(bk->hsnr[1]);
@@ -254,7 +254,7 @@ int cached_occupancy(spiir_bank* bk, bool g, size_t smem, int* occ)
 FilterParams base_params(const spiir_bank* bk)
 {
     FilterParams p{};
-    p.ar = bk->ar; p.ai2 = bk->ai2; p.b = bk->b; p.dly = bk->dly;
+    p.ar = bk->ar; p.ai = bk->ai; p.b = bk->b; p.dly = bk->dly;
     p.item_round0 = bk->item_round0; p.work = bk->work; p.n_items = bk->n_items;
     p.uniform_groups = bk->uniform_groups ? 1 : 0;
     p.canon = bk->canon;
@@ -292,7 +292,7 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
     CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kWarp * kStreamWarps, smem));
     if (occ < 1) return fail(SPIIR_ECUDA, "streaming kernel does not fit on an SM (smem %zu)", smem);
     StreamParams p{};
-    p.ar = bk->ar; p.ai2 = bk->ai2; p.b = bk->b; p.dly = bk->dly; p.y = bk->y;
+    p.ar = bk->ar; p.ai = bk->ai; p.b = bk->b; p.dly = bk->dly; p.y = bk->y;
     p.xwin = xwin; p.w0 = w0; p.n = (int32_t)n; p.n_tiles = bk->n_tiles; p.scratch = bk->stream_scratch;
     const int64_t ctas = std::min<int64_t>((bk->n_tiles + kStreamWarps - 1) / kStreamWarps, (int64_t)bk->n_sm * occ);
     void* args[] = {(void*)&p};
@@ -403,7 +403,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
         // carry scan: c_0 = y, c_{q+1} = a1^seg_len c_q + z_q   (double precision)
         const int threads = 256;
         const unsigned blocks = (unsigned)((bk->n_slots + threads - 1) / threads);
-        spiir_scan_carry_kernel<<<blocks, threads, 0, st>>>(bk->ar, bk->ai2, bk->y, bk->zbuf, bk->cbuf,
+        spiir_scan_carry_kernel<<<blocks, threads, 0, st>>>(bk->ar, bk->ai, bk->y, bk->zbuf, bk->cbuf,
                                                             bk->n_slots, (int32_t)n_seg, seg_len);
         g_launches.fetch_add(1, std::memory_order_relaxed);
         CU_TRY(cudaGetLastError());
@@ -569,6 +569,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         bk->NC = 1;
         for (int nc : {4, 2}) {
             if (stream) {                                   // sized for the streaming kernels (one big CTA per SM)
+                if (nc == 4) continue;                      // LDS.128 buys nothing there and costs registers
                 if (stream_smem_bytes(bk->F, nc, hist + kStreamMax, nullptr) <= bk->smem_optin &&
                     (hist + 2048) * 4 * nc <= room) { bk->NC = nc; break; }
                 continue;
@@ -596,7 +597,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->uniform_groups = L.uniform_groups;
     bk->multi_round = (L.work.size() / (size_t)bk->W) > (L.item_round0.size() - 1);
     if (e == cudaSuccess) e = upload(&bk->ar, L.ar);
-    if (e == cudaSuccess) e = upload(&bk->ai2, L.ai2);
+    if (e == cudaSuccess) e = upload(&bk->ai, L.ai);
     if (e == cudaSuccess) e = upload(&bk->b, L.b);
     if (e == cudaSuccess) e = upload(&bk->dly, L.dly);
     if (e == cudaSuccess) e = upload(&bk->item_round0, L.item_round0);

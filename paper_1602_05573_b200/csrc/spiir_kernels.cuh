@@ -50,7 +50,7 @@ __device__ __forceinline__ u64 ld_pair(const float* p) { return *reinterpret_cas
 struct FilterParams {
     // bank (slot order)
     const float* ar;        // [n_slots]
-    const float* ai2;       // [2 n_slots] (-a_im, a_im)
+    const float* ai;        // [n_slots] Im a1
     const float* b;         // [2 n_slots] (b_re, b_im)
     const int32_t* dly;     // [n_slots]
     // work list
@@ -377,7 +377,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
                 if (active) {
                     const int64_t s = ((int64_t)ww.tile * F + f) * kWarp + lane;
                     ar[f] = p.ar[s];
-                    AI[f] = ld_pair(p.ai2 + 2 * s);
+                    { const float a_im = p.ai[s]; AI[f] = pack2(-a_im, a_im); }
                     B[f] = ld_pair(p.b + 2 * s);
                     Y[f] = p.y_in ? ld_pair(p.y_in + (int64_t)seg * p.y_in_stride + 2 * s) : 0ull;
                     const int p0 = p.w0 - p.dly[s];            // window index of this filter's first input
@@ -480,7 +480,7 @@ constexpr int kStreamMax = 64;          // samples per call served by the stream
 __host__ __device__ constexpr int stream_warps(int F) { return F <= 4 ? 24 : 16; }
 
 struct StreamParams {
-    const float* ar; const float* ai2; const float* b; const int32_t* dly;
+    const float* ar; const float* ai; const float* b; const int32_t* dly;
     float* y;                     // state, updated in place
     const float* xwin; int32_t w0; int32_t n;
     int64_t n_tiles;
@@ -536,27 +536,27 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
         for (int f = 0; f < F; ++f) {
             const int64_t s = s0 + f * kWarp;
             ar[f] = p.ar[s];
-            AI[f] = ld_pair(p.ai2 + 2 * s);
+            { const float a_im = p.ai[s]; AI[f] = pack2(-a_im, a_im); }
             B[f] = ld_pair(p.b + 2 * s);
             Y[f] = ld_pair(p.y + 2 * s);
             const int p0 = p.w0 - p.dly[s];
             const int c = p0 & (NC - 1);
             xo[f] = (int)(c * cstride) + p0 - c;
         }
-        // Ask for the next tile of this warp now (its 8F cache lines, one or two per lane), so that its loads hit L1
+        // Ask for the next tile of this warp now (its 7F cache lines, one or two per lane), so that its loads hit L1
         // after this tile's arithmetic instead of waiting for HBM: the warps never have nothing in flight.
         if (tile + n_warps < p.n_tiles) {
             const int64_t t0n = (tile + n_warps) * F * kWarp;          // first slot of the next tile
 #pragma unroll
-            for (int q = 0; q < (8 * F + kWarp - 1) / kWarp; ++q) {
+            for (int q = 0; q < (7 * F + kWarp - 1) / kWarp; ++q) {
                 const int idx = lane + q * kWarp;
                 const float* line;
                 if (idx < F) line = p.ar + t0n + idx * kWarp;
-                else if (idx < 3 * F) line = p.ai2 + 2 * t0n + (idx - F) * kWarp;
-                else if (idx < 5 * F) line = p.b + 2 * t0n + (idx - 3 * F) * kWarp;
-                else if (idx < 6 * F) line = reinterpret_cast<const float*>(p.dly) + t0n + (idx - 5 * F) * kWarp;
-                else line = p.y + 2 * t0n + (idx - 6 * F) * kWarp;
-                if (idx < 8 * F) asm volatile("prefetch.global.L1 [%0];" ::"l"(line));
+                else if (idx < 2 * F) line = p.ai + t0n + (idx - F) * kWarp;
+                else if (idx < 4 * F) line = p.b + 2 * t0n + (idx - 2 * F) * kWarp;
+                else if (idx < 5 * F) line = reinterpret_cast<const float*>(p.dly) + t0n + (idx - 4 * F) * kWarp;
+                else line = p.y + 2 * t0n + (idx - 5 * F) * kWarp;
+                if (idx < 7 * F) asm volatile("prefetch.global.L1 [%0];" ::"l"(line));
             }
         }
         u64* row = p.scratch + tile * kStreamMax;
@@ -602,14 +602,14 @@ __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, con
 // zero-state end values z_p of segments p = 0..P-2 (all of length seg_len), produce the true start
 // states c_{p+1} = a1^seg_len * c_p + z_p.  Powers and the combine are evaluated in double from the
 // float32 a1 (SURVEY.md section 8(c) finding F2), then rounded once to float32.
-__global__ void spiir_scan_carry_kernel(const float* __restrict__ ar, const float* __restrict__ ai2,
+__global__ void spiir_scan_carry_kernel(const float* __restrict__ ar, const float* __restrict__ ai,
                                         const float* __restrict__ y, const float* __restrict__ z,
                                         float* __restrict__ c, int64_t n_slots, int32_t n_seg, int64_t seg_len)
 {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_slots) return;
     // a^L by binary exponentiation in double
-    double pr = 1.0, pi = 0.0, br = (double)ar[s], bi = (double)ai2[2 * s + 1];
+    double pr = 1.0, pi = 0.0, br = (double)ar[s], bi = (double)ai[s];
     for (int64_t e = seg_len; e > 0; e >>= 1) {
         if (e & 1) { const double tr = pr * br - pi * bi, ti = pr * bi + pi * br; pr = tr; pi = ti; }
         const double tr = br * br - bi * bi, ti = 2.0 * br * bi; br = tr; bi = ti;

@@ -37,7 +37,7 @@ struct HostLayout {
     int64_t n_tiles = 0;                // warp tiles
     int64_t n_slots = 0;                // n_tiles * F * 32
     std::vector<float> ar;              // [n_slots] Re a1
-    std::vector<float> ai2;             // [2*n_slots] (-Im a1, +Im a1) pairs for the packed complex FMA
+    std::vector<float> ai;              // [n_slots] Im a1 (the kernels build the (-Im, +Im) operand of the cross term)
     std::vector<float> b;               // [2*n_slots] (Re b0, Im b0)
     std::vector<int32_t> dly;           // [n_slots]
     std::vector<int64_t> slot_of_filter;  // [K] caller's filter index -> slot
@@ -180,7 +180,7 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
     L.n_tiles = tiles;
     L.n_slots = tiles * per_tile;
     L.ar.assign((size_t)L.n_slots, 0.f);
-    L.ai2.assign((size_t)L.n_slots * 2, 0.f);
+    L.ai.assign((size_t)L.n_slots, 0.f);
     L.b.assign((size_t)L.n_slots * 2, 0.f);
     L.dly.assign((size_t)L.n_slots, 0);
     L.slot_of_filter.assign((size_t)K, -1);
@@ -203,8 +203,7 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
                 if (i < Kt) {
                     const int64_t k = order[(size_t)i];
                     L.ar[s] = a1[2 * k];
-                    L.ai2[2 * s] = -a1[2 * k + 1];
-                    L.ai2[2 * s + 1] = a1[2 * k + 1];
+                    L.ai[s] = a1[2 * k + 1];
                     L.b[2 * s] = b0[2 * k];
                     L.b[2 * s + 1] = b0[2 * k + 1];
                     L.dly[s] = d[k];
@@ -225,8 +224,7 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
             for (size_t l = 0; l < groups[g].size(); ++l) {
                 const int64_t k = groups[g][l], s = slot0 + (int64_t)l;
                 L.ar[s] = a1[2 * k];
-                L.ai2[2 * s] = -a1[2 * k + 1];
-                L.ai2[2 * s + 1] = a1[2 * k + 1];
+                L.ai[s] = a1[2 * k + 1];
                 L.b[2 * s] = b0[2 * k];
                 L.b[2 * s + 1] = b0[2 * k + 1];
                 L.dly[s] = d[k];
