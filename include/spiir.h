@@ -45,7 +45,9 @@ enum {
     SPIIR_PATH_AUTO = 0,       /* choose per call from bank size and chunk length */
     SPIIR_PATH_THROUGHPUT = 1, /* filters across lanes, sequential in time, smem-staged window */
     SPIIR_PATH_SCAN = 2,       /* time-parallel: segments per filter + linear-recurrence carry scan */
-    SPIIR_PATH_STREAM = 3      /* tiny chunks, many filters: one pass over coefficients+state (HBM bound) */
+    SPIIR_PATH_STREAM = 3      /* tiny chunks, many filters (set at create): calls of <= 64 samples run as independent
+                                  warps + an ordered combine pass, one sweep over coefficients and state per call;
+                                  longer calls on the same bank use the blocked kernel */
 };
 
 typedef struct spiir_options {
