@@ -221,7 +221,7 @@ def test_cfg3_full_size_subset_and_invariants(env):
     pkg, oracle, torch = env
     inp = spiir_inputs.make_config(3)
     T = inp.n_templates
-    rows = spiir_inputs.parity_subset(T, 6, 3)
+    rows = spiir_inputs.parity_subset(T, 16, 3)
     # plant copies of checked templates at other positions: must come out bitwise equal to their originals
     src = rows[:3]
     dst = np.array([17, 2048, T - 2])
