@@ -301,6 +301,22 @@ def test_template_permutation_equivariance_and_determinism(env):
     assert np.array_equal(c.view(np.float32), a[perm].view(np.float32))      # rows permute bitwise
 
 
+def test_mbarrier_path_is_bitwise_reproducible(env):
+    # uniform bank -> the barrier-free hand-over between the warps of a template (no CTA-wide barrier): warps drift apart,
+    # the summation order must not
+    inp = spiir_inputs.make_config(3, n_templates=600, n_samples=8192)
+    rows = np.arange(0, 600, 7)
+    a = run_gpu(env, inp, chunks=[8192], path=1, rows=rows)
+    b = run_gpu(env, inp, chunks=[8192], path=1, rows=rows)
+    c = run_gpu(env, inp, chunks=[8192], path=1, F=8, rows=rows)      # 4 warps per template instead of 2
+    d = run_gpu(env, inp, chunks=[8192], path=1, F=8, rows=rows)
+    assert np.array_equal(a.view(np.float32), b.view(np.float32))
+    assert np.array_equal(c.view(np.float32), d.view(np.float32))
+    ref = env[1].run_inputs(inp.select_templates(rows[:8]))
+    check(a[:8], ref)
+    check(c[:8], ref)
+
+
 def test_checkpoint_resume(env):
     pkg, _, torch = env
     inp = spiir_inputs.make_random_bank(31, [300, 77], 2000, d_max=500)
