@@ -117,7 +117,8 @@ int spiir_filter_host(spiir_bank *bank, const float *x_host, int64_t n, float *s
 int spiir_filter_host_async(spiir_bank *bank, const float *x_host, int64_t n, float *snr_host, int64_t ld);
 int spiir_bank_host_sync(spiir_bank *bank);
 
-/* Zero the filter state and the input history (a cold bank again); enqueued on the stream. */
+/* Zero the filter state and the input history (a cold bank again); enqueued on the stream.  Waits first for chunks
+ * of spiir_filter_host_async that are still in flight. */
 int spiir_bank_reset(spiir_bank *bank, void *stream);
 
 /* Sizes.  Return -1 for a null handle. */

@@ -763,6 +763,10 @@ int spiir_bank_reset(spiir_bank* bk, void* stream)
     if (!bk) return fail(SPIIR_EINVAL, "null bank");
     cudaStream_t st = (cudaStream_t)stream;
     CU_TRY(cudaSetDevice(bk->device));
+    if (bk->free_pending[0] || bk->free_pending[1]) {      // chunks of the asynchronous host entry may still be in flight
+        int rc = spiir_bank_host_sync(bk);
+        if (rc) return rc;
+    }
     CU_TRY(cudaMemsetAsync(bk->y, 0, (size_t)std::max<int64_t>(bk->n_slots, 1) * 2 * sizeof(float), st));
     bk->pos = round_up(bk->D, 4);
     CU_TRY(cudaMemsetAsync(bk->tape[bk->cur], 0, (size_t)(bk->pos + 8) * sizeof(float), st));
