@@ -55,6 +55,22 @@ def measured_hbm_peak():
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
+def measured_body_ceiling():
+    """Fraction of the nominal FP32 peak the register file lets the 4-instruction filter body reach, measured now by the
+    committed microbenchmark (paper_1602_05573_b200/fp32_pipe_probe, built by build()); None if it is not built."""
+    import re
+    import subprocess
+    exe = ROOT / "paper_1602_05573_b200" / "fp32_pipe_probe"
+    if not exe.exists():
+        return None
+    try:
+        out = subprocess.run([str(exe), "1965"], capture_output=True, text=True, timeout=120).stdout
+        m = re.search(r"ceiling of the kernel by 12-flop accounting: ([0-9.]+) %", out)
+        return float(m.group(1)) / 100.0 if m else None
+    except Exception:
+        return None
+
+
 def workload_name(inp):
     return (f"{inp.name}: {inp.n_templates} templates x {inp.n_filters // max(inp.n_templates, 1)} filters (mean), "
             f"{inp.n_samples} samples, streaming in {inp.chunk}-sample chunks")
@@ -264,7 +280,9 @@ def run_ours(args):
                 "launches_per_call": launches_per_call, "call_ms": avg_call_s * 1e3,
                 "algorithmic_flop_per_launch": FLOPS_PER_FILTER_SAMPLE * fs_call / launches_per_call,
                 "algorithmic_hbm_bytes_per_launch": (8.0 * T * L + 36.0 * inp.n_filters * launches_per_call) / launches_per_call,
-                "reachable_frac_register_file": 0.599,   # profiles/r01_fp32_pipe_probe.md: the 4-instruction body alone
+                # what the register file lets the 4-instruction body alone reach (profiles/r01_fp32_pipe_probe.md: 0.599);
+                # re-measured below when the probe executable is built
+                "reachable_frac_register_file": 0.599,
                 "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1965 MHz (clocks.max.sm); no driver-measured FP32 peak exists",
                 "issue_slot_util": 8 * fs_call / avg_call_s / (N_SM * LANES * BOOST_HZ),
                 "hbm_write_gbs": 8.0 * T * L / avg_call_s / 1e9}
@@ -324,6 +342,11 @@ def run_ours(args):
                        "h2d_bytes_per_step": int(N * 4), "d2h_bytes_per_step": int(T * N * 8),
                        "steps": e2e_steps, "api": "spiir_filter_host_async per chunk + spiir_bank_host_sync per step (pinned host buffers)"}
 
+    if rank == 0 and world == 1 and roofline.get("bound") == "alu":
+        live = measured_body_ceiling()
+        if live is not None:
+            roofline["reachable_frac_register_file"] = live
+            roofline["reachable_frac_source"] = "fp32_pipe_probe, this run"
     # ---- the CPU oracle beside it (rank 0, N = 1 only): a reported baseline, not the target
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         r, dt, sub, cores = time_oracle(inp, args.cpu_templates)
