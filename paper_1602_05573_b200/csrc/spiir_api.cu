@@ -70,6 +70,8 @@ struct spiir_bank {
     int64_t* tile_begin = nullptr;   // [T+1] first warp tile of every template (streaming combine)
     u64* stream_scratch = nullptr;   // [n_tiles][kStreamMax] per-tile partial sums (streaming path)
     bool stream_configured = false;
+    int stream_occ = 0;
+    size_t stream_occ_smem = 0;
     u64* peaks = nullptr;            // [T] packed (power bits << 32 | ~index) of the running call (spiir_filter_peaks)
     float* peak_snr = nullptr;       // internal SNR rows for spiir_filter_peaks without an SNR buffer (multi-round templates)
     int64_t peak_snr_cap = 0;
@@ -288,9 +290,14 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
         CU_TRY(cudaMalloc((void**)&bk->stream_scratch, (size_t)std::max<int64_t>(bk->n_tiles, 1) * kStreamMax * sizeof(u64)));
     const int kStreamWarps = stream_warps(bk->F);
     const size_t smem = stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr);
-    int occ = 0;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kWarp * kStreamWarps, smem));
-    if (occ < 1) return fail(SPIIR_ECUDA, "streaming kernel does not fit on an SM (smem %zu)", smem);
+    if (bk->stream_occ_smem != smem) {          // one driver query per window size, not per call
+        int occ = 0;
+        CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kWarp * kStreamWarps, smem));
+        if (occ < 1) return fail(SPIIR_ECUDA, "streaming kernel does not fit on an SM (smem %zu)", smem);
+        bk->stream_occ = occ;
+        bk->stream_occ_smem = smem;
+    }
+    const int occ = bk->stream_occ;
     StreamParams p{};
     p.ar = bk->ar; p.ai = bk->ai; p.b = bk->b; p.dly = bk->dly; p.y = bk->y;
     p.xwin = xwin; p.w0 = w0; p.n = (int32_t)n; p.n_tiles = bk->n_tiles; p.scratch = bk->stream_scratch;
