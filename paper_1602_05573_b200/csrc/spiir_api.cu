@@ -351,7 +351,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     }
     if (n_seg <= 1) {
         // ------------------------------------------------ sequential-in-time path
-        bk->last_path = (path == SPIIR_PATH_STREAM) ? SPIIR_PATH_STREAM : SPIIR_PATH_THROUGHPUT;
+        bk->last_path = SPIIR_PATH_THROUGHPUT;
         int64_t sub = n;
         if (!gmem) {
             const int64_t sub_max = std::max<int64_t>(kTS, (max_win - w0) / kTS * kTS);
