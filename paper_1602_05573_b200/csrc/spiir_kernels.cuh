@@ -494,6 +494,24 @@ __host__ __device__ inline size_t stream_smem_bytes(int F, int NC, int64_t win_l
     return (size_t)(NC * cstride) * sizeof(float) + (size_t)stream_warps(F) * kTrWarp * sizeof(u64);
 }
 
+// The 7F cache lines of a warp tile's coefficients and state, one or two per lane, requested into L1.
+template <int F>
+__device__ __forceinline__ void stream_prefetch_tile(const StreamParams& p, int64_t tile, int lane)
+{
+    const int64_t t0n = tile * F * kWarp;          // first slot of the tile
+#pragma unroll
+    for (int q = 0; q < (7 * F + kWarp - 1) / kWarp; ++q) {
+        const int idx = lane + q * kWarp;
+        const float* line;
+        if (idx < F) line = p.ar + t0n + idx * kWarp;
+        else if (idx < 2 * F) line = p.ai + t0n + (idx - F) * kWarp;
+        else if (idx < 4 * F) line = p.b + 2 * t0n + (idx - 2 * F) * kWarp;
+        else if (idx < 5 * F) line = reinterpret_cast<const float*>(p.dly) + t0n + (idx - 4 * F) * kWarp;
+        else line = p.y + 2 * t0n + (idx - 5 * F) * kWarp;
+        if (idx < 7 * F) asm volatile("prefetch.global.L1 [%0];" ::"l"(line));
+    }
+}
+
 template <int F, int NC>
 __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kernel(const StreamParams p)
 {
@@ -504,6 +522,8 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
     const int win_len = p.w0 + p.n;
     int64_t cstride;
     stream_smem_bytes(F, NC, win_len, &cstride);
+    // the first tile's coefficients travel while the window is staged
+    if ((int64_t)blockIdx.x * kStreamWarps + warp < p.n_tiles) stream_prefetch_tile<F>(p, (int64_t)blockIdx.x * kStreamWarps + warp, lane);
     {
         const float4* src = reinterpret_cast<const float4*>(p.xwin);
         const int n4 = (int)(cstride / 4), v4 = (win_len + 3) / 4;
@@ -545,20 +565,7 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
         }
         // Ask for the next tile of this warp now (its 7F cache lines, one or two per lane), so that its loads hit L1
         // after this tile's arithmetic instead of waiting for HBM: the warps never have nothing in flight.
-        if (tile + n_warps < p.n_tiles) {
-            const int64_t t0n = (tile + n_warps) * F * kWarp;          // first slot of the next tile
-#pragma unroll
-            for (int q = 0; q < (7 * F + kWarp - 1) / kWarp; ++q) {
-                const int idx = lane + q * kWarp;
-                const float* line;
-                if (idx < F) line = p.ar + t0n + idx * kWarp;
-                else if (idx < 2 * F) line = p.ai + t0n + (idx - F) * kWarp;
-                else if (idx < 4 * F) line = p.b + 2 * t0n + (idx - 2 * F) * kWarp;
-                else if (idx < 5 * F) line = reinterpret_cast<const float*>(p.dly) + t0n + (idx - 4 * F) * kWarp;
-                else line = p.y + 2 * t0n + (idx - 5 * F) * kWarp;
-                if (idx < 7 * F) asm volatile("prefetch.global.L1 [%0];" ::"l"(line));
-            }
-        }
+        if (tile + n_warps < p.n_tiles) stream_prefetch_tile<F>(p, tile + n_warps, lane);
         u64* row = p.scratch + tile * kStreamMax;
 #pragma unroll 1
         for (int tt = 0; tt < p.n; tt += kTT) {
