@@ -117,7 +117,10 @@ __device__ __forceinline__ void tile_step(const float* __restrict__ xs, const in
                     unpack2(Y[f], yr, yi);
                     t = ffma2(AI[f], pack2(yi, yr), t);
                     Y[f] = ffma2(pack2(ar[f], ar[f]), Y[f], t);
-                    S[j] = (f == 0) ? Y[f] : fadd2(S[j], Y[f]);
+                    // S_j = ((Y_0 + Y_1) + Y_2) + ...: the first two outputs are added directly, no copy of Y_0
+                    if (F == 1) S[j] = Y[0];
+                    else if (f == 1) S[j] = fadd2(Y[0], Y[1]);
+                    else if (f > 1) S[j] = fadd2(S[j], Y[f]);
                 }
             } else {
                 S[j] = 0ull;
