@@ -63,8 +63,7 @@ struct spiir_bank {
     double avg_conflict_degree = 0.0;
     spiir_options opt{};
     // device bank
-    float *ar = nullptr, *ai = nullptr, *b = nullptr, *y = nullptr;
-    int32_t* dly = nullptr;
+    float *coef = nullptr, *y = nullptr;   // per-tile coefficient records (spiir_layout.hpp), filter state
     int32_t* item_round0 = nullptr;
     int32_t* canon = nullptr;
     int64_t* tile_begin = nullptr;   // [T+1] first warp tile of every template (streaming combine)
@@ -113,7 +112,7 @@ int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 void free_bank(spiir_bank* bk)
 {
     if (!bk) return;
-    cudaFree(bk->ar); cudaFree(bk->ai); cudaFree(bk->b); cudaFree(bk->y); cudaFree(bk->dly);
+    cudaFree(bk->coef); cudaFree(bk->y);
     cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->tile_begin); cudaFree(bk->stream_scratch); cudaFree(bk->peaks); cudaFree(bk->peak_snr); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
     cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
     cudaFree(bk->hx); cudaFree(bk->hsnr[0]); cudaFree(bk->hsnr[1]);
@@ -256,7 +255,7 @@ int cached_occupancy(spiir_bank* bk, bool g, size_t smem, int* occ)
 FilterParams base_params(const spiir_bank* bk)
 {
     FilterParams p{};
-    p.ar = bk->ar; p.ai = bk->ai; p.b = bk->b; p.dly = bk->dly;
+    p.coef = bk->coef;
     p.item_round0 = bk->item_round0; p.work = bk->work; p.n_items = bk->n_items;
     p.uniform_groups = bk->uniform_groups ? 1 : 0;
     p.canon = bk->canon;
@@ -299,7 +298,7 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
     }
     const int occ = bk->stream_occ;
     StreamParams p{};
-    p.ar = bk->ar; p.ai = bk->ai; p.b = bk->b; p.dly = bk->dly; p.y = bk->y;
+    p.coef = bk->coef; p.y = bk->y;
     p.xwin = xwin; p.w0 = w0; p.n = (int32_t)n; p.n_tiles = bk->n_tiles; p.scratch = bk->stream_scratch;
     const int64_t ctas = std::min<int64_t>((bk->n_tiles + kStreamWarps - 1) / kStreamWarps, (int64_t)bk->n_sm * occ);
     void* args[] = {(void*)&p};
@@ -410,7 +409,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
         // carry scan: c_0 = y, c_{q+1} = a1^seg_len c_q + z_q   (double precision)
         const int threads = 256;
         const unsigned blocks = (unsigned)((bk->n_slots + threads - 1) / threads);
-        spiir_scan_carry_kernel<<<blocks, threads, 0, st>>>(bk->ar, bk->ai, bk->y, bk->zbuf, bk->cbuf,
+        spiir_scan_carry_kernel<<<blocks, threads, 0, st>>>(bk->coef, (int32_t)bk->F, bk->y, bk->zbuf, bk->cbuf,
                                                             bk->n_slots, (int32_t)n_seg, seg_len);
         g_launches.fetch_add(1, std::memory_order_relaxed);
         CU_TRY(cudaGetLastError());
@@ -603,10 +602,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bk->avg_conflict_degree = L.avg_conflict_degree;
     bk->uniform_groups = L.uniform_groups;
     bk->multi_round = (L.work.size() / (size_t)bk->W) > (L.item_round0.size() - 1);
-    if (e == cudaSuccess) e = upload(&bk->ar, L.ar);
-    if (e == cudaSuccess) e = upload(&bk->ai, L.ai);
-    if (e == cudaSuccess) e = upload(&bk->b, L.b);
-    if (e == cudaSuccess) e = upload(&bk->dly, L.dly);
+    if (e == cudaSuccess) e = upload(&bk->coef, L.coef);
     if (e == cudaSuccess) e = upload(&bk->item_round0, L.item_round0);
     if (e == cudaSuccess) e = upload(&bk->work, L.work);
     if (e == cudaSuccess) e = upload(&bk->canon, L.canon);

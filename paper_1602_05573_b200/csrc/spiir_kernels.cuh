@@ -49,10 +49,7 @@ __device__ __forceinline__ u64 ld_pair(const float* p) { return *reinterpret_cas
 
 struct FilterParams {
     // bank (slot order)
-    const float* ar;        // [n_slots]
-    const float* ai;        // [n_slots] Im a1
-    const float* b;         // [2 n_slots] (b_re, b_im)
-    const int32_t* dly;     // [n_slots]
+    const float* coef;      // [n_tiles][5 F x 32] per-tile coefficient records: ar | ai | (b_re, b_im) | delay bits
     // work list
     const int32_t* item_round0;   // [n_items + 1]
     const WarpWork* work;         // [n_rounds * W]
@@ -379,11 +376,12 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
             for (int f = 0; f < F; ++f) {
                 if (active) {
                     const int64_t s = ((int64_t)ww.tile * F + f) * kWarp + lane;
-                    ar[f] = p.ar[s];
-                    { const float a_im = p.ai[s]; AI[f] = pack2(-a_im, a_im); }
-                    B[f] = ld_pair(p.b + 2 * s);
+                    const float* rec = p.coef + (int64_t)ww.tile * (5 * F * kWarp) + f * kWarp + lane;
+                    ar[f] = rec[0];
+                    { const float a_im = rec[F * kWarp]; AI[f] = pack2(-a_im, a_im); }
+                    B[f] = ld_pair(rec + 2 * F * kWarp + f * kWarp + lane);
                     Y[f] = p.y_in ? ld_pair(p.y_in + (int64_t)seg * p.y_in_stride + 2 * s) : 0ull;
-                    const int p0 = p.w0 - p.dly[s];            // window index of this filter's first input
+                    const int p0 = p.w0 - __float_as_int(rec[4 * F * kWarp]);   // window index of this filter's first input
                     const int c = p0 & (NC - 1);               // the copy in which p0 is aligned
                     xo[f] = (int)(c * cstride) + p0 - c;
                 } else {
@@ -483,7 +481,7 @@ constexpr int kStreamMax = 64;          // samples per call served by the stream
 __host__ __device__ constexpr int stream_warps(int F) { return F <= 4 ? 24 : 16; }
 
 struct StreamParams {
-    const float* ar; const float* ai; const float* b; const int32_t* dly;
+    const float* coef;            // per-tile coefficient records (see FilterParams)
     float* y;                     // state, updated in place
     const float* xwin; int32_t w0; int32_t n;
     int64_t n_tiles;
@@ -501,16 +499,12 @@ __host__ __device__ inline size_t stream_smem_bytes(int F, int NC, int64_t win_l
 template <int F>
 __device__ __forceinline__ void stream_prefetch_tile(const StreamParams& p, int64_t tile, int lane)
 {
-    const int64_t t0n = tile * F * kWarp;          // first slot of the tile
+    const float* rec = p.coef + tile * (5 * F * kWarp);    // 5F consecutive lines of coefficients
+    const float* st = p.y + 2 * tile * F * kWarp;          // 2F consecutive lines of state
 #pragma unroll
     for (int q = 0; q < (7 * F + kWarp - 1) / kWarp; ++q) {
         const int idx = lane + q * kWarp;
-        const float* line;
-        if (idx < F) line = p.ar + t0n + idx * kWarp;
-        else if (idx < 2 * F) line = p.ai + t0n + (idx - F) * kWarp;
-        else if (idx < 4 * F) line = p.b + 2 * t0n + (idx - 2 * F) * kWarp;
-        else if (idx < 5 * F) line = reinterpret_cast<const float*>(p.dly) + t0n + (idx - 4 * F) * kWarp;
-        else line = p.y + 2 * t0n + (idx - 5 * F) * kWarp;
+        const float* line = idx < 5 * F ? rec + idx * kWarp : st + (idx - 5 * F) * kWarp;
         if (idx < 7 * F) asm volatile("prefetch.global.L1 [%0];" ::"l"(line));
     }
 }
@@ -558,11 +552,12 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
 #pragma unroll
         for (int f = 0; f < F; ++f) {
             const int64_t s = s0 + f * kWarp;
-            ar[f] = p.ar[s];
-            { const float a_im = p.ai[s]; AI[f] = pack2(-a_im, a_im); }
-            B[f] = ld_pair(p.b + 2 * s);
+            const float* rec = p.coef + tile * (5 * F * kWarp) + f * kWarp + lane;
+            ar[f] = rec[0];
+            { const float a_im = rec[F * kWarp]; AI[f] = pack2(-a_im, a_im); }
+            B[f] = ld_pair(rec + 2 * F * kWarp + f * kWarp + lane);
             Y[f] = ld_pair(p.y + 2 * s);
-            const int p0 = p.w0 - p.dly[s];
+            const int p0 = p.w0 - __float_as_int(rec[4 * F * kWarp]);
             const int c = p0 & (NC - 1);
             xo[f] = (int)(c * cstride) + p0 - c;
         }
@@ -612,14 +607,16 @@ __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, con
 // zero-state end values z_p of segments p = 0..P-2 (all of length seg_len), produce the true start
 // states c_{p+1} = a1^seg_len * c_p + z_p.  Powers and the combine are evaluated in double from the
 // float32 a1 (SURVEY.md section 8(c) finding F2), then rounded once to float32.
-__global__ void spiir_scan_carry_kernel(const float* __restrict__ ar, const float* __restrict__ ai,
+__global__ void spiir_scan_carry_kernel(const float* __restrict__ coef, int32_t F,
                                         const float* __restrict__ y, const float* __restrict__ z,
                                         float* __restrict__ c, int64_t n_slots, int32_t n_seg, int64_t seg_len)
 {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_slots) return;
     // a^L by binary exponentiation in double
-    double pr = 1.0, pi = 0.0, br = (double)ar[s], bi = (double)ai[s];
+    const int64_t per_tile = (int64_t)F * kWarp;
+    const float* rec = coef + (s / per_tile) * 5 * per_tile + s % per_tile;
+    double pr = 1.0, pi = 0.0, br = (double)rec[0], bi = (double)rec[per_tile];
     for (int64_t e = seg_len; e > 0; e >>= 1) {
         if (e & 1) { const double tr = pr * br - pi * bi, ti = pr * bi + pi * br; pr = tr; pi = ti; }
         const double tr = br * br - bi * bi, ti = 2.0 * br * bi; br = tr; bi = ti;

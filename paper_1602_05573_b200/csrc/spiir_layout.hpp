@@ -16,6 +16,7 @@
 #pragma once
 #include <algorithm>
 #include <cstdint>
+#include <cstring>
 #include <numeric>
 #include <vector>
 
@@ -40,6 +41,10 @@ struct HostLayout {
     std::vector<float> ai;              // [n_slots] Im a1 (the kernels build the (-Im, +Im) operand of the cross term)
     std::vector<float> b;               // [2*n_slots] (Re b0, Im b0)
     std::vector<int32_t> dly;           // [n_slots]
+    // The device copy of the coefficients: one contiguous record per warp tile,
+    //   [ar: F x 32][ai: F x 32][b: F x 32 (re, im) pairs][delay: F x 32 as int bits]  = 5 F x 32 floats,
+    // so that a warp reaches everything it needs for a tile from one base address (5 F consecutive cache lines).
+    std::vector<float> coef;
     std::vector<int64_t> slot_of_filter;  // [K] caller's filter index -> slot
     std::vector<int64_t> tile_begin;    // [T+1] first tile of each template
     // work list: items (one CTA at a time), each with >= 1 rounds of W warp entries
@@ -298,6 +303,22 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
         }
     }
     flush();
+    L.coef.assign((size_t)L.n_tiles * 5 * per_tile, 0.f);
+    for (int64_t tile = 0; tile < L.n_tiles; ++tile) {
+        float* rec = L.coef.data() + (size_t)tile * 5 * per_tile;
+        for (int64_t r = 0; r < per_tile; ++r) {
+            const int64_t sl = tile * per_tile + r;
+            rec[r] = L.ar[(size_t)sl];
+            rec[per_tile + r] = L.ai[(size_t)sl];
+            rec[2 * per_tile + 2 * r] = L.b[(size_t)(2 * sl)];
+            rec[2 * per_tile + 2 * r + 1] = L.b[(size_t)(2 * sl + 1)];
+            int32_t dl = L.dly[(size_t)sl];
+            float bits;
+            static_assert(sizeof(bits) == sizeof(dl), "delay is stored as int bits in a float slot");
+            memcpy(&bits, &dl, sizeof(bits));
+            rec[4 * per_tile + r] = bits;
+        }
+    }
     // Named per-template barriers are only safe when a warp position always belongs to the same group shape:
     // otherwise a fast warp could enter a hardware barrier that a slower group of another shape still uses.
     {
