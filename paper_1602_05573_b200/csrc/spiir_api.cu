@@ -277,7 +277,15 @@ const void* select_stream_kernel(int F, int NC)
     return nullptr;
 }
 
-int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st, u64* peaks)
+bool stream_applies(const spiir_bank* bk, int w0, int64_t n)
+{
+    return bk->opt.path == SPIIR_PATH_STREAM && n <= kStreamMax && !bk->gmem_only && select_stream_kernel(bk->F, bk->NC) &&
+           stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr) <= bk->smem_optin;
+}
+
+// xnew != nullptr: the chunk is not on the tape yet; the kernel reads it from xnew and CTA 0 appends it at `append`.
+int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st, u64* peaks,
+               const float* xnew = nullptr, float* append = nullptr)
 {
     const void* fn = select_stream_kernel(bk->F, bk->NC);
     if (!fn) return fail(SPIIR_EINVAL, "no streaming kernel for F=%d NC=%d", bk->F, bk->NC);
@@ -287,6 +295,7 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
     }
     if (!bk->stream_scratch)
         CU_TRY(cudaMalloc((void**)&bk->stream_scratch, (size_t)std::max<int64_t>(bk->n_tiles, 1) * kStreamMax * sizeof(u64)));
+    u64* scratch = bk->stream_scratch;
     const int kStreamWarps = stream_warps(bk->F);
     const size_t smem = stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr);
     if (bk->stream_occ_smem != smem) {          // one driver query per window size, not per call
@@ -299,10 +308,25 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
     const int occ = bk->stream_occ;
     StreamParams p{};
     p.coef = bk->coef; p.y = bk->y;
-    p.xwin = xwin; p.w0 = w0; p.n = (int32_t)n; p.n_tiles = bk->n_tiles; p.scratch = bk->stream_scratch;
+    p.xwin = xwin; p.w0 = w0; p.n = (int32_t)n; p.n_tiles = bk->n_tiles; p.scratch = scratch;
+    p.xnew = xnew; p.append = append;
     const int64_t ctas = std::min<int64_t>((bk->n_tiles + kStreamWarps - 1) / kStreamWarps, (int64_t)bk->n_sm * occ);
-    void* args[] = {(void*)&p};
-    CU_TRY(cudaLaunchKernel(fn, dim3((unsigned)ctas, 1, 1), dim3(kWarp * kStreamWarps, 1, 1), args, smem, st));
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    {
+        // programmatic dependent launch: the grid is set up and the first tile requested while the previous kernel in the
+        // stream (normally the previous call's combine pass) drains; the kernel waits for it before it reads anything else
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)ctas, 1, 1);
+        cfg.blockDim = dim3(kWarp * kStreamWarps, 1, 1);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        void* args[] = {(void*)&p};
+        CU_TRY(cudaLaunchKernelExC(&cfg, fn, args));
+    }
     const int64_t total = bk->T * n;
     {
         // programmatic dependent launch: the combine grid is set up while the streaming kernel drains and waits
@@ -312,12 +336,9 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
         cfg.blockDim = dim3(256, 1, 1);
         cfg.dynamicSmemBytes = 0;
         cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        CU_TRY(cudaLaunchKernelEx(&cfg, spiir_stream_combine_kernel, (const u64*)bk->stream_scratch,
+        CU_TRY(cudaLaunchKernelEx(&cfg, spiir_stream_combine_kernel, (const u64*)scratch,
                                   (const int64_t*)bk->tile_begin, (int32_t)bk->T, (int32_t)n, snr, ld, peaks));
     }
     g_launches.fetch_add(2, std::memory_order_relaxed);
@@ -334,9 +355,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     const int64_t max_win = ((int64_t)smem_cap - (int64_t)fixed_smem(bk->F, bk->W)) / (4 * bk->NC) - 48;
     const bool gmem = bk->gmem_only;          // history alone does not fit: read x through L1/L2
     int path = bk->opt.path;
-    if (path == SPIIR_PATH_STREAM && n <= kStreamMax && !gmem && select_stream_kernel(bk->F, bk->NC) &&
-        stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr) <= smem_cap)
-        return run_stream(bk, xwin, w0, n, snr, ld, st, peaks);
+    if (stream_applies(bk, w0, n)) return run_stream(bk, xwin, w0, n, snr, ld, st, peaks);
     // ---- how much time-parallelism is needed to fill the machine?  The scan path does the recurrence twice, so it
     // only pays when the bank leaves at least half of the SMs idle (cfg2: 128 items on 148 SMs run 1.7x faster
     // sequentially).
@@ -633,10 +652,16 @@ int filter_impl(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, i
     int rc = ensure_tape(bk, n, st);
     if (rc) return rc;
     float* tape = bk->tape[bk->cur];
-    CU_TRY(cudaMemcpyAsync(tape + bk->pos, x_dev, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st));
     const int64_t start_al = (bk->pos - bk->D) / 4 * 4;
     const int w0 = (int)(bk->pos - start_al);
-    rc = run_chunk(bk, tape + start_al, w0, n, snr_dev, ld, st, peaks);
+    if (stream_applies(bk, w0, n)) {
+        // tiny chunk: no separate copy (it would sit between the kernels and break their launch chain); the kernel stages
+        // history + chunk itself and appends the chunk to the tape
+        rc = run_stream(bk, tape + start_al, w0, n, snr_dev, ld, st, peaks, x_dev, tape + bk->pos);
+    } else {
+        CU_TRY(cudaMemcpyAsync(tape + bk->pos, x_dev, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        rc = run_chunk(bk, tape + start_al, w0, n, snr_dev, ld, st, peaks);
+    }
     if (rc) { bk->poisoned = true; return rc; }
     bk->pos += n;
     return SPIIR_OK;

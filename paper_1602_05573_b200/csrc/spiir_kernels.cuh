@@ -483,7 +483,9 @@ __host__ __device__ constexpr int stream_warps(int F) { return F <= 4 ? 24 : 16;
 struct StreamParams {
     const float* coef;            // per-tile coefficient records (see FilterParams)
     float* y;                     // state, updated in place
-    const float* xwin; int32_t w0; int32_t n;
+    const float* xwin; int32_t w0; int32_t n;   // history: xwin[0 .. w0) (16-byte aligned); the n new samples follow it ...
+    const float* xnew;            // ... unless xnew != nullptr: then they are read from the caller's chunk xnew[0 .. n)
+    float* append;                // where CTA 0 stores the chunk for later calls (the bank's tape); nullptr: already there
     int64_t n_tiles;
     u64* scratch;                 // [n_tiles][kStreamMax] partial sums of every warp tile
 };
@@ -521,11 +523,28 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
     stream_smem_bytes(F, NC, win_len, &cstride);
     // the first tile's coefficients travel while the window is staged
     if ((int64_t)blockIdx.x * kStreamWarps + warp < p.n_tiles) stream_prefetch_tile<F>(p, (int64_t)blockIdx.x * kStreamWarps + warp, lane);
+    // Launched with programmatic dependent launch: the grid is set up and the first coefficients are requested while the
+    // previous kernel in the stream (normally the previous call's combine pass) is still running.  Everything read from
+    // here on may have been written by that kernel's predecessors or by the caller's own kernels: wait for them.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     {
         const float4* src = reinterpret_cast<const float4*>(p.xwin);
         const int n4 = (int)(cstride / 4), v4 = (win_len + 3) / 4;
         for (int i = tid; i < n4; i += kThreads) {
-            const float4 v = i < v4 ? src[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (i < v4) {
+                if (!p.xnew || 4 * i + 3 < p.w0) {
+                    v = src[i];
+                } else {                               // the float4 that straddles history and chunk, and the chunk itself
+                    float e[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int k = 4 * i + q;
+                        e[q] = k < p.w0 ? p.xwin[k] : (k < win_len ? p.xnew[k - p.w0] : 0.f);
+                    }
+                    v = make_float4(e[0], e[1], e[2], e[3]);
+                }
+            }
             reinterpret_cast<float4*>(smem)[i] = v;
             if (NC > 1) {
                 const float e[4] = {v.x, v.y, v.z, v.w};
@@ -542,6 +561,9 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
     const float* xs = smem;
     u64* mytr = reinterpret_cast<u64*>(smem + NC * cstride) + (size_t)warp * kTrWarp;
     __syncthreads();
+    // the chunk joins the history for later calls (every CTA has staged its window: nobody reads the tape beyond w0)
+    if (p.append && p.xnew && blockIdx.x == 0)
+        for (int i = tid; i < p.n; i += kThreads) p.append[i] = p.xnew[i];
 
     const int64_t n_warps = (int64_t)gridDim.x * kStreamWarps;
     for (int64_t tile = (int64_t)blockIdx.x * kStreamWarps + warp; tile < p.n_tiles; tile += n_warps) {
@@ -589,6 +611,7 @@ __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, con
     const int32_t t = (int32_t)(i / n), j = (int32_t)(i % n);
     const int64_t t0 = tile_begin[t], t1 = tile_begin[t + 1];
     asm volatile("griddepcontrol.wait;" ::: "memory");     // launched early (PDL): the streaming kernel's rows from here on
+    asm volatile("griddepcontrol.launch_dependents;");     // the next call's streaming kernel may be set up (it waits itself)
     u64 acc = scratch[t0 * kStreamMax + j];
     // loads 16 tiles ahead of the (ordered) additions: the chain of adds is short, the chain of L2 latencies is not
     for (int64_t tile = t0 + 1; tile < t1; tile += 16) {
