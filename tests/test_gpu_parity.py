@@ -3,6 +3,7 @@ seeded float32 inputs.  Acceptance (BASELINE.json:north_star): per template
     max_n |SNR_gpu - SNR_ref| <= 1e-4 * max_n |SNR_ref|
 for one-shot and for every chunked run; the dyadic golden vector P7 must match bitwise.
 """
+import os
 from fractions import Fraction
 from pathlib import Path
 
@@ -440,3 +441,42 @@ def test_filter_peaks_cfg3_blocking_and_exact_tie(env):
             pkg.spiir_filter_peaks(bank.handle, x[64:], power, index)
             torch.cuda.synchronize()
             assert power.item() == 0.0 and index.item() == 0
+
+
+# ------------------------------------------------------------------ seeded fuzz over shapes, paths and blockings
+@pytest.mark.parametrize("seed", range(int(os.environ.get("SPIIR_FUZZ_SEEDS", "24"))))
+def test_fuzz_shapes_paths_blockings(env, seed):
+    pkg, oracle, torch = env
+    rng = np.random.default_rng(1000 + seed)
+    n_t = int(rng.integers(1, 13))
+    kind = seed % 4
+    if kind == 0:
+        counts = rng.integers(1, 40, n_t)                   # tiny templates
+    elif kind == 1:
+        counts = rng.integers(1, 700, n_t)                  # mixed
+    elif kind == 2:
+        counts = np.full(n_t, int(rng.choice([64, 128, 256, 512])))   # uniform (mbarrier hand-over path)
+    else:
+        counts = np.exp(rng.uniform(np.log(1), np.log(3000), n_t)).astype(int) + 1
+    d_max = int(rng.choice([0, 1, 31, 200, 1500, 5000]))
+    n = int(rng.integers(1, 2500))
+    inp = spiir_inputs.make_random_bank(2000 + seed, counts.tolist(), n, d_max=d_max)
+    ref = oracle.run_inputs(inp)
+    chunks, left = [], n
+    while left > 0:
+        c = int(min(left, rng.choice([0, 1, 7, 16, 63, 64, 65, 300, 1024, 2500])))
+        chunks.append(c)
+        left -= c
+    path = int(rng.integers(0, 4))
+    F = int(rng.choice([0, 0, 1, 2, 4, 8, 16]))
+    small = int(rng.integers(0, 3))
+    if path == 3 and F not in (0, 4, 8):
+        F = 0
+    if small == 1 and F not in (0, 8):
+        F = 0
+    got = run_gpu(env, inp, chunks=chunks, path=path, F=F, small=small)
+    err = check(got, ref)
+    assert err <= TOL, (seed, counts.tolist(), d_max, chunks, path, F, small)
+    if seed % 3 == 0:                                           # the fused trigger reduction on the same case
+        opt = pkg.SpiirOptions(path=path, filters_per_thread=F, small_templates=small)
+        check_peaks(pkg, torch, oracle, inp, [c for c in chunks if c > 0], opt, bool(seed % 2), ref)
