@@ -9,9 +9,14 @@ with state carry), i.e. 16 spiir_filter calls = 1.0995e12 filter-samples.  Input
 timed region starts (`value`); `e2e` repeats the measurement through spiir_filter_host_async / spiir_bank_host_sync with host buffers
 (H2D of every chunk and D2H of every SNR block inside the timed region).  Prints ONE JSON line.
 
+The default run (N = 1, --config 3) also times every other config of BASELINE.json in short legs and reports them
+under `per_config` (cfg0, cfg1 one-shot and 16 x 4096, cfg2, cfg4: filter-samples/s, roofline fraction, per-call
+p50/p99, path taken, clocks of that leg); --no-per-config skips them.
+
 N > 1 (torchrun, one rank per GPU): templates are independent, so every rank filters
 its own seeded 4096-template bank -- no data-path collective -- and `value` is the total over ranks divided by
-the slowest rank's time ("scaling": "weak").
+the slowest rank's time ("scaling": "weak").  With --shard ONE bank is split over the ranks by template
+(shard_templates, longest-processing-time bin packing; "scaling": "strong"; per-rank filter counts in `shard`).
 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores, on a bounded sample of the
 same workload; rank 0 only.
@@ -53,22 +58,6 @@ def measured_hbm_peak():
         return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
     except Exception:
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
-
-
-def measured_body_ceiling():
-    """Fraction of the nominal FP32 peak the register file lets the 4-instruction filter body reach, measured now by the
-    committed microbenchmark (paper_1602_05573_b200/fp32_pipe_probe, built by build()); None if it is not built."""
-    import re
-    import subprocess
-    exe = ROOT / "paper_1602_05573_b200" / "fp32_pipe_probe"
-    if not exe.exists():
-        return None
-    try:
-        out = subprocess.run([str(exe), "1965"], capture_output=True, text=True, timeout=120).stdout
-        m = re.search(r"ceiling of the kernel by 12-flop accounting: ([0-9.]+) %", out)
-        return float(m.group(1)) / 100.0 if m else None
-    except Exception:
-        return None
 
 
 def workload_name(inp):
@@ -166,7 +155,8 @@ def run_reference(args):
     return 0
 
 
-def run_ours(args):
+def setup(args):
+    """Device, process group and library for this rank -> (torch, dist, pkg, world, rank, dev_index, red_dev, oversubscribed)."""
     import torch
     import torch.distributed as dist
     import paper_1602_05573_b200 as pkg
@@ -178,8 +168,8 @@ def run_ours(args):
         raise SystemExit("bench.py needs a CUDA device: the SPIIR library has no CPU fallback")
     n_dev = torch.cuda.device_count()
     # fewer GPUs than ranks (or SPIIR_BENCH_BACKEND=gloo): a functional check of the multi-rank path only -- NCCL cannot put
-    # two ranks on one GPU, so the timing exchange then goes over gloo on the host
-    oversubscribed = world > 1 and (local_rank >= n_dev or os.environ.get("SPIIR_BENCH_BACKEND") == "gloo")
+    # two ranks on one GPU, so the timing exchange then goes over gloo on the host and the line says "functional_only"
+    oversubscribed = world > 1 and (world > n_dev or os.environ.get("SPIIR_BENCH_BACKEND") == "gloo")
     dev_index = local_rank % n_dev
     torch.cuda.set_device(dev_index)
     red_dev = "cpu" if oversubscribed else "cuda"
@@ -198,17 +188,35 @@ def run_ours(args):
             while not pkg.library_path().exists() and time.time() - t_wait < 600:
                 time.sleep(1.0)
     pkg.load_library()
+    return torch, dist, pkg, world, rank, dev_index, red_dev, oversubscribed
 
-    # every rank filters its own seeded bank of the config's size (weak scaling, no exchange step)
-    inp = spiir_inputs.make_config(args.config)
-    if rank > 0:
-        rng = np.random.default_rng(spiir_inputs.SEED0 + 1000 * rank + args.config)
-        perm = rng.permutation(inp.n_templates)
-        inp = inp.select_templates(perm)               # same distributions, different bank per rank
-    N, L, T = inp.n_samples, inp.chunk, inp.n_templates
-    if args.path == 0 and L <= 64 and inp.n_filters >= (1 << 20):
-        args.path = pkg.PATH_STREAM            # tiny chunks over a large bank: the HBM-bound streaming blocking
-    opt = pkg.SpiirOptions(path=args.path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta,
+
+def measure(ctx, args, cfg, steps, warmup, *, chunk=None, e2e=False, label=None):
+    """Time `steps` steps of configs[cfg] on this rank's GPU (a step = the config's whole streaming run; chunk=0: one call
+    over the whole series).  -> dict with value, ms_per_step, roofline, latency, clocks, launches, path (+ e2e)."""
+    torch, dist, pkg, world, rank, dev_index, red_dev, oversubscribed = ctx
+    inp = spiir_inputs.make_config(cfg)
+    shard_info = None
+    if args.shard and world > 1:
+        # ONE bank split over the ranks by template (DESIGN.md section 9; SURVEY.md section 8(e)): longest-processing-time
+        # bin packing on the filter counts, no data-path collective, every rank filters the same strain
+        parts = pkg.shard_templates(inp.offsets, world)
+        kt = np.diff(inp.offsets)
+        loads = [int(kt[p_].sum()) for p_ in parts]
+        shard_info = {"filters_per_rank": loads, "templates_per_rank": [int(p_.size) for p_ in parts],
+                      "imbalance_max_over_mean": max(loads) / (sum(loads) / world)}
+        total_filters = inp.n_filters
+        inp = inp.select_templates(parts[rank])
+    elif rank > 0:
+        # weak scaling: every rank filters its own seeded bank of the config's size (same distributions, another bank)
+        rng = np.random.default_rng(spiir_inputs.SEED0 + 1000 * rank + cfg)
+        inp = inp.select_templates(rng.permutation(inp.n_templates))
+    N, T = inp.n_samples, inp.n_templates
+    L = inp.chunk if chunk is None else (N if chunk == 0 else chunk)
+    path = args.path
+    if path == 0 and L <= 64 and inp.n_filters >= (1 << 20):
+        path = pkg.PATH_STREAM            # tiny chunks over a large bank: the HBM-bound streaming blocking
+    opt = pkg.SpiirOptions(path=path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta,
                            window_copies=args.window_copies, scan_segments=args.scan_segments)
     bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, dev_index, opt)
     x = torch.from_numpy(inp.x).cuda()
@@ -239,7 +247,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         one_step()
     barrier()
     launches0 = pkg.spiir_kernel_launches()
@@ -247,14 +255,14 @@ def run_ours(args):
     with ClockSampler(dev_index) as clocks:
         barrier()
         start.record(stream)
-        for s in range(args.steps):
+        for s in range(steps):
             one_step()                      # the timed region carries no per-call events: they would sit between the
         stop.record(stream)                 # kernels of consecutive calls and break their programmatic launch chain
         barrier()
     launches = pkg.spiir_kernel_launches() - launches0
     elapsed_ms = start.elapsed_time(stop)
     # per-call latency: a separate pass with one event pair per call (at most 2 steps' worth of calls)
-    lat_steps = min(args.steps, 2)
+    lat_steps = min(steps, 2 if n_calls > 64 else 50)
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(n_calls + 1)] for _ in range(lat_steps)]
     for s in range(lat_steps):
         one_step(ev[s])
@@ -265,19 +273,23 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     elapsed_ms_max = float(t.item())
     fs_step = inp.filter_samples
-    value = world * fs_step * args.steps / (elapsed_ms_max * 1e-3)
+    if shard_info is not None:
+        value = total_filters * N * steps / (elapsed_ms_max * 1e-3)      # one bank over all ranks: strong scaling
+        shard_info["rank0_ms_per_step"] = elapsed_ms / steps
+    else:
+        value = world * fs_step * steps / (elapsed_ms_max * 1e-3)
 
-    # dominant kernel: spiir_filter_kernel, one launch per spiir_filter call (the call also enqueues one
-    # 64 KB device-to-device append of the chunk, < 0.1 % of the call)
+    # dominant kernel: spiir_filter_kernel (1 or 2 launches per spiir_filter call; the call also enqueues one device-to-
+    # device append of the chunk, < 0.1 % of the call)
     fs_call = inp.n_filters * L
-    avg_call_s = elapsed_ms * 1e-3 / (args.steps * n_calls)      # timed region (includes the reset of each step)
+    avg_call_s = elapsed_ms * 1e-3 / (steps * n_calls)      # timed region (includes the reset of each step)
     achieved_tflops = FLOPS_PER_FILTER_SAMPLE * fs_call / avg_call_s / 1e12
-    launches_per_call = max(1.0, launches / float(args.steps * n_calls))      # kernel launches of one spiir_filter call
+    launches_per_call = max(1.0, launches / float(steps * n_calls))      # kernel launches of one spiir_filter call
     traffic = args.ncu_traffic_bytes
     default_blocking = not (args.filters_per_thread or args.warps_per_cta or args.window_copies or args.path)
-    if traffic is None and args.config == 3 and default_blocking:
+    if traffic is None and cfg == 3 and default_blocking and chunk is None:
         traffic = NCU_TRAFFIC_CFG3_LAUNCH
-    if traffic is None and args.config == 4 and not (args.filters_per_thread or args.warps_per_cta or args.window_copies):
+    if traffic is None and cfg == 4 and not (args.filters_per_thread or args.warps_per_cta or args.window_copies) and chunk is None:
         traffic = NCU_TRAFFIC_CFG4_LAUNCH
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved_tflops / FP32_PEAK_TFLOPS, "traffic": traffic,
@@ -285,9 +297,6 @@ def run_ours(args):
                 "launches_per_call": launches_per_call, "call_ms": avg_call_s * 1e3,
                 "algorithmic_flop_per_launch": FLOPS_PER_FILTER_SAMPLE * fs_call / launches_per_call,
                 "algorithmic_hbm_bytes_per_launch": (8.0 * T * L + 36.0 * inp.n_filters * launches_per_call) / launches_per_call,
-                # what the register file lets the 4-instruction body alone reach (profiles/r01_fp32_pipe_probe.md: 0.599);
-                # re-measured below when the probe executable is built
-                "reachable_frac_register_file": 0.599,
                 "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1965 MHz (clocks.max.sm); no driver-measured FP32 peak exists",
                 "issue_slot_util": 8 * fs_call / avg_call_s / (N_SM * LANES * BOOST_HZ),
                 "hbm_write_gbs": 8.0 * T * L / avg_call_s / 1e9}
@@ -302,23 +311,22 @@ def run_ours(args):
         peak_gbs, peak_src = measured_hbm_peak()
         roofline = {"bound": "hbm", "achieved": bytes_call / avg_call_s / 1e9, "peak": peak_gbs, "unit": "GB/s",
                     "frac": bytes_call / avg_call_s / 1e9 / peak_gbs, "traffic": traffic,
-                    "kernel": "spiir_stream_kernel (+ spiir_stream_combine_kernel)", "launch_ms": avg_call_s * 1e3 / launches_per_call,
+                    "kernel": "spiir_stream_kernel", "launch_ms": avg_call_s * 1e3 / launches_per_call,
                     "launches_per_call": launches_per_call, "call_ms": avg_call_s * 1e3, "peak_source": peak_src,
                     "algorithmic_bytes_per_call": bytes_call}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": elapsed_ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_name(inp), "path": bank.last_path,
-                       "l2": "each step writes %.2f GB of SNR and reads a %.0f MB bank: working set larger than the 126 MB L2"
-                             % (T * N * 8 / 1e9, inp.n_filters * 28 / 1e6),
-                       "snr_buffer": "whole [T][N]" if keep_whole else "per-chunk [T][L] reused",
-                       "entry": ["spiir_filter", "spiir_filter_peaks (no SNR output)", "spiir_filter_peaks (+ SNR output)"][args.peaks]},
-            "pct_of_fp32_fma_peak": 100.0 * FLOPS_PER_FILTER_SAMPLE * value / world / (FP32_PEAK_TFLOPS * 1e12),
-            "gpu_launches": int(launches), "roofline": roofline, "latency": latency, "clocks": clocks.summary()}
+    res = {"workload": (label or workload_name(inp)) if chunk is None else f"{inp.name}: {T} templates, {N} samples, {n_calls} call(s) of {L}",
+           "value": value, "unit": UNIT, "steps": steps, "ms_per_step": elapsed_ms_max / steps, "path": bank.last_path,
+           "pct_of_fp32_fma_peak": 100.0 * FLOPS_PER_FILTER_SAMPLE * (value / world) / (FP32_PEAK_TFLOPS * 1e12),
+           "gpu_launches": int(launches), "roofline": roofline, "latency": latency, "clocks": clocks.summary(),
+           "snr_buffer": "whole [T][N]" if keep_whole else "per-chunk [T][L] reused",
+           "l2": "each step writes %.2f GB of SNR and reads a %.0f MB bank" % (T * N * 8 / 1e9, inp.n_filters * 28 / 1e6),
+           "_inp": inp}
+    if shard_info is not None:
+        res["shard"] = shard_info
 
     # ---- end to end through the public host-buffer entry (H2D + kernels + D2H inside the timed region)
-    if not args.no_e2e:
+    if e2e:
         xh = torch.from_numpy(inp.x).pin_memory()
         outh = torch.empty((2, T, L), dtype=torch.complex64).pin_memory()      # results land here, two chunks deep
         xh_np, outh_np = xh.numpy(), outh.numpy()
@@ -334,7 +342,7 @@ def run_ours(args):
 
         e2e_step()
         barrier()
-        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        e2e_steps = max(1, min(steps, args.e2e_steps))
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             e2e_step()
@@ -343,21 +351,67 @@ def run_ours(args):
         tt = torch.tensor([dt], dtype=torch.float64, device=red_dev)
         if world > 1:
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        line["e2e"] = {"value": world * fs_step * e2e_steps / float(tt.item()), "unit": UNIT,
-                       "h2d_bytes_per_step": int(N * 4), "d2h_bytes_per_step": int(T * N * 8),
-                       "steps": e2e_steps, "api": "spiir_filter_host_async per chunk + spiir_bank_host_sync per step (pinned host buffers)"}
+        fs_total = (total_filters * N) if shard_info is not None else world * fs_step
+        res["e2e"] = {"value": fs_total * e2e_steps / float(tt.item()), "unit": UNIT,
+                      "h2d_bytes_per_step": int(N * 4), "d2h_bytes_per_step": int(T * N * 8),
+                      "steps": e2e_steps, "api": "spiir_filter_host_async per chunk + spiir_bank_host_sync per step (pinned host buffers)"}
+        if keep_whole and not args.peaks:
+            # the last chunk's host block must equal the device-resident run of the same chunking bit for bit
+            c0 = (n_calls - 1) * L
+            n = N - c0
+            dev_last = snr[:, c0:c0 + n].cpu().numpy()
+            res["e2e"]["last_chunk_bitwise_equal_to_device_run"] = bool(
+                np.array_equal(outh_np[(n_calls - 1) & 1, :, :n].view(np.float32), dev_last.view(np.float32)))
+    bank.close()
+    del snr, x
+    torch.cuda.empty_cache()
+    return res
 
-    if rank == 0 and world == 1 and roofline.get("bound") == "alu":
-        live = measured_body_ceiling()
-        if live is not None:
-            roofline["reachable_frac_register_file"] = live
-            roofline["reachable_frac_source"] = "fp32_pipe_probe, this run"
+
+def run_ours(args):
+    ctx = setup(args)
+    torch, dist, pkg, world, rank, dev_index, red_dev, oversubscribed = ctx
+    main = measure(ctx, args, args.config, args.steps, args.warmup, e2e=not args.no_e2e)
+    inp = main.pop("_inp")
+    line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": main["ms_per_step"], "higher_is_better": True,
+            "scaling": "strong" if (args.shard and world > 1) else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": main["workload"], "path": main["path"],
+                       "l2": main["l2"] + ": working set larger than the 126 MB L2", "snr_buffer": main["snr_buffer"],
+                       "entry": ["spiir_filter", "spiir_filter_peaks (no SNR output)", "spiir_filter_peaks (+ SNR output)"][args.peaks]},
+            "pct_of_fp32_fma_peak": main["pct_of_fp32_fma_peak"],
+            "gpu_launches": main["gpu_launches"], "roofline": main["roofline"], "latency": main["latency"],
+            "clocks": main["clocks"]}
+    if "e2e" in main:
+        line["e2e"] = main["e2e"]
+    if "shard" in main:
+        line["shard"] = main["shard"]
+    if oversubscribed:
+        line["functional_only"] = True          # ranks share a GPU: the value is not a multi-GPU number
+        line["oversubscribed"] = True
+
+    # ---- every other config of BASELINE.json, driver-timed in the same run (N = 1 only; short legs)
+    if world == 1 and not args.no_per_config and args.config == 3:
+        per = {}
+        legs = [("cfg0", 0, None, 200), ("cfg1_oneshot", 1, 0, 20), ("cfg1_chunked", 1, None, 10), ("cfg2", 2, None, 5),
+                ("cfg4", 4, None, 2)]
+        for name, cfg, chunk, steps in legs:
+            r = measure(ctx, args, cfg, steps, 3, chunk=chunk)
+            r.pop("_inp")
+            rf = r["roofline"]
+            per[name] = {"workload": r["workload"], "value": r["value"], "unit": UNIT, "steps": steps, "ms_per_step": r["ms_per_step"],
+                         "path": r["path"], "bound": rf["bound"], "achieved": rf["achieved"], "peak": rf["peak"],
+                         "roofline_unit": rf["unit"], "frac": rf["frac"], "launches_per_call": rf["launches_per_call"],
+                         "p50_us": r["latency"]["p50_us"], "p99_us": r["latency"]["p99_us"],
+                         "call_us_back_to_back": rf["call_ms"] * 1e3, "samples_per_call": r["latency"]["samples_per_call"],
+                         "clocks": r["clocks"]}
+        line["per_config"] = per
+
     # ---- the CPU oracle beside it (rank 0, N = 1 only): a reported baseline, not the target
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         r, dt, sub, cores = time_oracle(inp, args.cpu_templates)
         line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
-                                "sample": f"first {sub.n_templates} of {T} templates, all {N} samples, {L}-sample chunks"}
-    bank.close()
+                                "sample": f"first {sub.n_templates} of {inp.n_templates} templates, all {inp.n_samples} samples, {inp.chunk}-sample chunks"}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -382,6 +436,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config legs (cfg0, cfg1, cfg2, cfg4) of the default run")
+    ap.add_argument("--shard", action="store_true", help="N > 1: split ONE bank over the ranks by template (strong scaling)")
     ap.add_argument("--cpu-templates", type=int, default=96, help="templates of the bounded oracle sample")
     ap.add_argument("--ref-templates", type=int, default=32, help="templates per step of --impl reference")
     ap.add_argument("--ncu-traffic-bytes", type=float, default=None,

@@ -18,8 +18,24 @@
  * Every step of the path runs in the library's own CUDA kernels (sm_100a).  There is no CPU fallback:
  * without a CUDA device every call that needs one fails with SPIIR_ECUDA.
  *
- * Threading: a handle is not thread-safe; distinct handles are.  Work is enqueued on the caller's
- * stream and is ordered with respect to it; calls return without synchronising the host unless noted.
+ * Threading and streams: a handle is not thread-safe; distinct handles are.  Work is enqueued on the caller's
+ * stream and is ordered with respect to it.  The calls that touch a bank's state (spiir_filter, spiir_filter_peaks,
+ * spiir_filter_host[_async], spiir_bank_reset, spiir_bank_get_state, spiir_bank_set_state) are also ordered among
+ * themselves in the order they are issued, whatever streams they name: a call that arrives on another stream than
+ * its predecessor makes its stream wait for an event recorded behind the predecessor's work (so alternating streams is
+ * safe, and costs one event per switch; calls that stay on one stream put nothing between their kernels).  The
+ * caller's own buffers (x_dev, snr_dev, ...) are ordered only by the stream they are used on.
+ * Host synchronisation and allocation: calls return without synchronising the host, except
+ *   - spiir_bank_create / spiir_bank_destroy (synchronise the device),
+ *   - spiir_filter_host and spiir_bank_host_sync (by contract),
+ *   - spiir_filter / spiir_filter_peaks when n exceeds every earlier call AND the 65 536 samples the input tape is
+ *     created for: the tape is then reallocated (cudaMalloc + one stream synchronisation),
+ *   - the first streaming-path call (one cudaMalloc of the per-tile scratch) and the first spiir_filter_peaks (one
+ *     cudaMalloc of [T] keys),
+ *   - spiir_filter_peaks with snr_dev == NULL on a bank with templates of more than 8 warp tiles, whenever n exceeds
+ *     every earlier such call (private SNR rows are reallocated: cudaMalloc + one stream synchronisation),
+ *   - spiir_filter_host_async when n exceeds every earlier call (staging buffers are reallocated).
+ * Every call makes the bank's device current for its duration and restores the caller's current device on return.
  */
 #ifndef SPIIR_H
 #define SPIIR_H
@@ -56,13 +72,16 @@ typedef struct spiir_options {
     int32_t filters_per_thread; /* 0 = choose; else 1, 2, 4, 8 or 16 (register blocking of the throughput kernel) */
     int32_t scan_segments;      /* 0 = choose; else time segments per call for SPIIR_PATH_SCAN */
     int32_t warps_per_cta;      /* 0 = choose; else 8, 16 or 32; valid (filters_per_thread, warps_per_cta) pairs:
-                                   (16,8) (8,8) (8,16) (4,8) (4,16) (4,32) (2,32) (1,32) */
+                                   (16,8) (8,8) (8,16) (4,8) (4,16) (4,32) (2,32) (1,32).  spiir_bank_create returns
+                                   SPIIR_EINVAL for any other pair; when only one of the two is given the other follows
+                                   it.  SPIIR_PATH_STREAM banks use 8 warps unless told otherwise, hence
+                                   filters_per_thread 4, 8 or 16 there */
     int32_t window_copies;      /* 0 = choose; else 1, 2 or 4 shifted copies of the input window in shared memory
                                    (= floats per shared-memory load); falls back if they do not fit */
     int32_t small_templates;    /* templates of <= 128 filters sharing warp tiles (sub-warp segments):
                                    0 = choose, 1 = on (forces the (8,16) blocking), 2 = off.  Not used with
                                    SPIIR_PATH_STREAM. */
-    int32_t reserved[1];        /* must be 0 */
+    int32_t reserved[1];        /* must be 0 (checked) */
 } spiir_options;
 
 /* Build a bank.  All pointers are HOST pointers; the arrays are copied, the caller keeps ownership.
@@ -135,7 +154,8 @@ int spiir_bank_set_state(spiir_bank *bank, const float *y_dev, const float *hist
 int spiir_bank_destroy(spiir_bank *bank);
 
 /* Host-only diagnostic (no CUDA call): lay the bank out exactly as spiir_bank_create would for the given
- * register blocking (filters_per_thread F in {2,4,8,16}, warps_per_cta W, window_copies NC in {1,2,4}) and
+ * register blocking (filters_per_thread F in {1,2,4,8,16}, warps_per_cta W: a valid pair, see spiir_options;
+ * window_copies NC in {1,2,4}) and
  * report it.  slot_of_filter (nullable, [K] int64, HOST) receives the device slot of every caller filter;
  * stats (nullable, [8] double, HOST) receives {n_slots, n_warp_tiles, n_cta_items, n_rounds,
  * avg_conflict_degree (mean over load phases of the largest number of lanes on one bank group; 1 = conflict

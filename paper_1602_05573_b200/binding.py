@@ -123,6 +123,16 @@ def spiir_bank_create(filter_offsets, a1, b0, delays, device: int = 0, options: 
     return h
 
 
+def _check_rows(bank, snr, *others):
+    """Marshalling checks only: the output tensors must have one row / entry per template and live on x's device."""
+    T = int(load_library().spiir_bank_num_templates(bank))
+    if snr is not None and (snr.dim() != 2 or snr.shape[0] != T):
+        raise ValueError(f"snr must have one row per template ({T}), got shape {tuple(snr.shape)}")
+    for name, t in others:
+        if t is not None and t.numel() != T:
+            raise ValueError(f"{name} must have one entry per template ({T}), got {t.numel()}")
+
+
 def spiir_filter(bank, x, snr, ld: int | None = None, stream=None, n: int | None = None):
     """x: CUDA float32 tensor [n]; snr: CUDA complex64 tensor whose row t starts ``ld`` elements after row t-1
     (a [T, ld] tensor, or a column slice ``big[:, c0:c0+n]`` of one).  Enqueues on ``stream``."""
@@ -131,6 +141,9 @@ def spiir_filter(bank, x, snr, ld: int | None = None, stream=None, n: int | None
         raise ValueError("x must be a contiguous CUDA float32 tensor")
     if snr.dtype != torch.complex64 or not snr.is_cuda:
         raise ValueError("snr must be a CUDA complex64 tensor")
+    if snr.device != x.device:
+        raise ValueError("x and snr must be on the same device (the bank's)")
+    _check_rows(bank, snr)
     n = int(x.numel()) if n is None else int(n)
     if ld is None:
         if snr.dim() != 2 or (snr.shape[1] > 1 and snr.stride(1) != 1) or snr.shape[1] < n:
@@ -148,6 +161,10 @@ def spiir_filter_peaks(bank, x, power=None, index=None, snr=None, stream=None):
     for name, t, dt in (("power", power, torch.float32), ("index", index, torch.int32)):
         if t is not None and (t.dtype != dt or not t.is_cuda or not t.is_contiguous()):
             raise ValueError(f"{name} must be a contiguous CUDA {dt} tensor")
+    for t in (power, index, snr):
+        if t is not None and t.device != x.device:
+            raise ValueError("x, power, index and snr must be on the same device (the bank's)")
+    _check_rows(bank, snr, ("power", power), ("index", index))
     n, ld, snr_ptr = int(x.numel()), int(x.numel()), None
     if snr is not None:
         if snr.dtype != torch.complex64 or not snr.is_cuda or snr.dim() != 2 or snr.shape[1] < n or \
@@ -165,6 +182,12 @@ def spiir_filter_host(bank, x: np.ndarray, snr: np.ndarray | None = None, asynch
     """Host-buffer entry: x float32 [n] numpy -> complex64 [T, n] numpy (H2D, kernels, D2H inside).
     ``asynchronous`` = spiir_filter_host_async: x and snr must be pinned and stay untouched until spiir_bank_host_sync."""
     lib = load_library()
+    if asynchronous:
+        # the copy is still reading x when this returns: a converted temporary would be freed under it
+        if not isinstance(x, np.ndarray) or x.dtype != np.float32 or x.ndim != 1 or not x.flags.c_contiguous:
+            raise ValueError("asynchronous: x must already be a C-contiguous float32 array (pinned), no conversion is made")
+        if snr is None:
+            raise ValueError("asynchronous: pass the (pinned) snr buffer the results are written to")
     x = np.ascontiguousarray(x, dtype=np.float32)
     T = int(lib.spiir_bank_num_templates(bank))
     if snr is None:

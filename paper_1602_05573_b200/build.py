@@ -15,21 +15,6 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC,-O3,-Wall", "-shared", "-cudart", "shared"]
 
 
-PROBE_SRC = CSRC / "fp32_pipe_probe.cu"
-PROBE_BIN = PKG / "fp32_pipe_probe"          # standalone microbenchmark behind the roofline ceiling in DESIGN.md section 7.1
-
-
-def build_probe(force: bool = False) -> Path:
-    """nvcc the FP32 pipe probe (run it on a B200: ``paper_1602_05573_b200/fp32_pipe_probe 1965``)."""
-    if force or not PROBE_BIN.exists() or PROBE_SRC.stat().st_mtime > PROBE_BIN.stat().st_mtime:
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = PROBE_BIN.with_suffix(f".tmp{os.getpid()}")
-        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-                        "-o", str(tmp), str(PROBE_SRC)], check=True)
-        os.replace(tmp, PROBE_BIN)
-    return PROBE_BIN
-
-
 def needs_build() -> bool:
     if not LIB.exists():
         return True
@@ -49,4 +34,3 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
-    print(build_probe(force="--force" in sys.argv))

@@ -39,6 +39,22 @@ int fail(int code, const char* fmt, ...)
                         cudaGetErrorString(e_));                                                  \
     } while (0)
 
+// Every entry switches to the bank's device and restores the caller's current device on return (a single-process
+// multi-GPU program must not find its current device changed by a library call).
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != device) err = cudaSetDevice(device);
+        else prev = -1;                      // nothing to restore
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 template <typename T>
 cudaError_t upload(T** dst, const std::vector<T>& v)
 {
@@ -90,7 +106,12 @@ struct spiir_bank {
     float* hsnr[2] = {nullptr, nullptr};
     int64_t hx_cap = 0, hsnr_cap = 0;
     cudaStream_t hstream = nullptr, cstream = nullptr;
-    cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_reset = nullptr;
+    cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+    // stream ordering: the bank's state (y, tape) is touched by one call after the other; when a call arrives on another
+    // stream than its predecessor's, that stream first waits for an event recorded behind the predecessor's work
+    cudaStream_t last_stream = nullptr;
+    bool last_stream_valid = false;
+    cudaEvent_t ev_order = nullptr;
     bool free_pending[2] = {false, false};
     int64_t host_piece = 0;          // pieces enqueued so far by the host-buffer entry (ping-pong index)
     // device facts
@@ -120,10 +141,24 @@ void free_bank(spiir_bank* bk)
         if (bk->ev_done[i]) cudaEventDestroy(bk->ev_done[i]);
         if (bk->ev_free[i]) cudaEventDestroy(bk->ev_free[i]);
     }
-    if (bk->ev_reset) cudaEventDestroy(bk->ev_reset);
+    if (bk->ev_order) cudaEventDestroy(bk->ev_order);
     if (bk->hstream) cudaStreamDestroy(bk->hstream);
     if (bk->cstream) cudaStreamDestroy(bk->cstream);
     delete bk;
+}
+
+// The bank's state is about to be used on stream st: order st behind the stream of the previous call if it differs.
+// Calls that stay on one stream (the normal case) cost nothing and put nothing between their kernels.
+int order_after_previous(spiir_bank* bk, cudaStream_t st)
+{
+    if (bk->last_stream_valid && bk->last_stream != st) {
+        if (!bk->ev_order) CU_TRY(cudaEventCreateWithFlags(&bk->ev_order, cudaEventDisableTiming));
+        CU_TRY(cudaEventRecord(bk->ev_order, bk->last_stream));
+        CU_TRY(cudaStreamWaitEvent(st, bk->ev_order, 0));
+    }
+    bk->last_stream = st;
+    bk->last_stream_valid = true;
+    return SPIIR_OK;
 }
 
 // (re)allocate the tape so that a chunk of n samples fits behind the history; keeps the history
@@ -134,14 +169,22 @@ int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
     const int64_t hist0 = round_up(bk->D, 4);
     if (bk->cap < need) {
         const int64_t cap = round_up(bk->D, 4) + std::max<int64_t>(4 * n, 1 << 16) + 16;
+        // growing the tape allocates and synchronises the stream (documented in spiir.h: only calls longer than any
+        // before, beyond the 65 536 samples the tape is created for)
         float* nt[2] = {nullptr, nullptr};
-        for (int i = 0; i < 2; ++i) CU_TRY(cudaMalloc((void**)&nt[i], (size_t)cap * sizeof(float)));
-        CU_TRY(cudaMemsetAsync(nt[0], 0, (size_t)cap * sizeof(float), st));
-        CU_TRY(cudaMemsetAsync(nt[1], 0, (size_t)cap * sizeof(float), st));
-        if (bk->tape[bk->cur] && bk->D > 0)
-            CU_TRY(cudaMemcpyAsync(nt[0] + hist0 - bk->D, bk->tape[bk->cur] + bk->pos - bk->D,
-                                   (size_t)bk->D * sizeof(float), cudaMemcpyDeviceToDevice, st));
-        CU_TRY(cudaStreamSynchronize(st));
+        cudaError_t e = cudaMalloc((void**)&nt[0], (size_t)cap * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&nt[1], (size_t)cap * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemsetAsync(nt[0], 0, (size_t)cap * sizeof(float), st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(nt[1], 0, (size_t)cap * sizeof(float), st);
+        if (e == cudaSuccess && bk->tape[bk->cur] && bk->D > 0)
+            e = cudaMemcpyAsync(nt[0] + hist0 - bk->D, bk->tape[bk->cur] + bk->pos - bk->D,
+                                (size_t)bk->D * sizeof(float), cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) {
+            cudaFree(nt[0]);
+            cudaFree(nt[1]);
+            return fail(e == cudaErrorMemoryAllocation ? SPIIR_ENOMEM : SPIIR_ECUDA, "input tape: %s", cudaGetErrorString(e));
+        }
         cudaFree(bk->tape[0]);
         cudaFree(bk->tape[1]);
         bk->tape[0] = nt[0];
@@ -545,22 +588,15 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         if (o.window_copies != 0 && o.window_copies != 1 && o.window_copies != 2 && o.window_copies != 4)
             return fail(SPIIR_EINVAL, "window_copies must be 0, 1, 2 or 4");
         if (o.small_templates < 0 || o.small_templates > 2) return fail(SPIIR_EINVAL, "small_templates must be 0, 1 or 2");
+        if (opt->struct_size >= (int32_t)sizeof(spiir_options) && o.reserved[0] != 0)
+            return fail(SPIIR_EINVAL, "spiir_options.reserved must be 0");
     }
-    int n_dev = 0;
-    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0)
-        return fail(SPIIR_ECUDA, "no CUDA device available (this library has no CPU fallback)");
-    if (device < 0 || device >= n_dev) return fail(SPIIR_EINVAL, "device %d out of range", device);
-    CU_TRY(cudaSetDevice(device));
-
-    spiir_bank* bk = new (std::nothrow) spiir_bank();
-    if (!bk) return fail(SPIIR_ENOMEM, "out of host memory");
-    bk->device = device;
-    bk->opt = o;
-    bk->T = T; bk->K = K; bk->D = D;
+    // ---- blocking: F filters per thread, W warps per CTA, shared tiles or not (host logic, no device needed)
     const bool stream = (o.path == SPIIR_PATH_STREAM);     // tiny chunks: small CTAs, several per SM
     double plain_cost = 0;
-    bk->F = stream && !o.filters_per_thread ? 4 : choose_F(T, off, o.filters_per_thread, &plain_cost);
-    bk->W = o.warps_per_cta ? o.warps_per_cta : (stream ? 8 : default_warps(bk->F));
+    int F = stream && !o.filters_per_thread ? 4 : choose_F(T, off, o.filters_per_thread, &plain_cost);
+    int W = o.warps_per_cta ? o.warps_per_cta : (stream ? 8 : default_warps(F));
+    bool segmented = false;
     // Small templates (<= 128 filters) can share warp tiles (PAPER.md:L333-L335 size-aware mapping):
     // blocking F = 8 / 16 warps.  Taken when asked for, or by itself when its estimated cost is lower.
     if (!stream && o.small_templates != 2 && (o.filters_per_thread == 0 || o.filters_per_thread == 8) &&
@@ -574,9 +610,44 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
             packed += w < kWarp ? kSharedTileCost * (double)(w * 8) : slot_cost(8) * (double)((Kt + 255) / 256 * 256);
         }
         if (any_small && (o.small_templates == 1 || packed < plain_cost)) {
-            bk->F = 8; bk->W = 16; bk->segmented = true;
+            F = 8; W = 16; segmented = true;
         }
     }
+    // The (filters_per_thread, warps_per_cta) pair must be one a compiled kernel serves: checked here, not at the first
+    // spiir_filter.  When only one of the two was requested the other follows it.
+    if (!segmented && !valid_blocking(F, W)) {
+        if (o.filters_per_thread && o.warps_per_cta)
+            return fail(SPIIR_EINVAL, "unsupported blocking: filters_per_thread %d with warps_per_cta %d%s", F, W,
+                        stream ? " (SPIIR_PATH_STREAM banks use 8 warps by default: filters_per_thread 4, 8 or 16)" : "");
+        if (o.warps_per_cta) {               // W fixed: the largest F that pairs with it
+            int f_ok = 0;
+            for (int f : {16, 8, 4, 2, 1})
+                if (valid_blocking(f, W)) { f_ok = f; break; }
+            F = f_ok;
+        } else if (stream) {                 // F fixed, W = 8 comes with the streaming path
+            return fail(SPIIR_EINVAL, "SPIIR_PATH_STREAM serves filters_per_thread 4, 8 or 16 (got %d)", F);
+        } else {
+            W = default_warps(F);
+        }
+        if (!valid_blocking(F, W))
+            return fail(SPIIR_EINVAL, "unsupported blocking: filters_per_thread %d with warps_per_cta %d", F, W);
+    }
+    if (segmented && !select_kernel(F, W, 1, false, false, true))
+        return fail(SPIIR_EINVAL, "shared tiles of small templates need the (8, 16) blocking");
+
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0)
+        return fail(SPIIR_ECUDA, "no CUDA device available (this library has no CPU fallback)");
+    if (device < 0 || device >= n_dev) return fail(SPIIR_EINVAL, "device %d out of range", device);
+    DeviceGuard dg(device);
+    CU_TRY(dg.err);
+
+    spiir_bank* bk = new (std::nothrow) spiir_bank();
+    if (!bk) return fail(SPIIR_ENOMEM, "out of host memory");
+    bk->device = device;
+    bk->opt = o;
+    bk->T = T; bk->K = K; bk->D = D;
+    bk->F = F; bk->W = W; bk->segmented = segmented;
     cudaDeviceProp prop;
     cudaError_t e = cudaGetDeviceProperties(&prop, device);
     if (e != cudaSuccess) {
@@ -648,8 +719,11 @@ namespace {
 // spiir_filter and spiir_filter_peaks: append the chunk to the tape, run the kernels, advance the tape.
 int filter_impl(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, int64_t ld, cudaStream_t st, u64* peaks)
 {
-    CU_TRY(cudaSetDevice(bk->device));
-    int rc = ensure_tape(bk, n, st);
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
+    int rc = order_after_previous(bk, st);
+    if (rc) return rc;
+    rc = ensure_tape(bk, n, st);
     if (rc) return rc;
     float* tape = bk->tape[bk->cur];
     const int64_t start_al = (bk->pos - bk->D) / 4 * 4;
@@ -690,10 +764,16 @@ int spiir_filter_peaks(spiir_bank* bk, const float* x_dev, int64_t n, float* snr
     if (!x_dev || (!power_dev && !index_dev)) return fail(SPIIR_EINVAL, "null device pointer");
     if (n > (int64_t)1 << 30) return fail(SPIIR_EINVAL, "chunk too long");
     cudaStream_t st = (cudaStream_t)stream;
-    CU_TRY(cudaSetDevice(bk->device));
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
+    {
+        int rc0 = order_after_previous(bk, st);
+        if (rc0) return rc0;
+    }
     if (!bk->peaks) CU_TRY(cudaMalloc((void**)&bk->peaks, (size_t)bk->T * sizeof(u64)));
     if (!snr_dev && bk->multi_round) {
         // templates that span several CTA rounds accumulate their sums through SNR rows: give them private ones
+        // (allocates and synchronises the stream the first time and whenever n grows: documented in spiir.h)
         if (bk->peak_snr_cap < bk->T * n) {
             CU_TRY(cudaStreamSynchronize(st));
             cudaFree(bk->peak_snr); bk->peak_snr = nullptr; bk->peak_snr_cap = 0;
@@ -718,11 +798,11 @@ int spiir_filter_host_async(spiir_bank* bk, const float* x_host, int64_t n, floa
     if (n < 0 || ld < n) return fail(SPIIR_EINVAL, "need 0 <= n <= ld");
     if (n == 0) return SPIIR_OK;
     if (!x_host || !snr_host) return fail(SPIIR_EINVAL, "null host pointer");
-    CU_TRY(cudaSetDevice(bk->device));
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
     if (!bk->hstream) {
         CU_TRY(cudaStreamCreateWithFlags(&bk->hstream, cudaStreamNonBlocking));
         CU_TRY(cudaStreamCreateWithFlags(&bk->cstream, cudaStreamNonBlocking));
-        CU_TRY(cudaEventCreateWithFlags(&bk->ev_reset, cudaEventDisableTiming));
         for (int i = 0; i < 2; ++i) {
             CU_TRY(cudaEventCreateWithFlags(&bk->ev_done[i], cudaEventDisableTiming));
             CU_TRY(cudaEventCreateWithFlags(&bk->ev_free[i], cudaEventDisableTiming));
@@ -772,7 +852,8 @@ int spiir_bank_host_sync(spiir_bank* bk)
 {
     if (!bk) return fail(SPIIR_EINVAL, "null bank");
     if (!bk->hstream) return SPIIR_OK;
-    CU_TRY(cudaSetDevice(bk->device));
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
     CU_TRY(cudaStreamSynchronize(bk->hstream));
     CU_TRY(cudaStreamSynchronize(bk->cstream));
     bk->free_pending[0] = bk->free_pending[1] = false;
@@ -790,18 +871,19 @@ int spiir_bank_reset(spiir_bank* bk, void* stream)
 {
     if (!bk) return fail(SPIIR_EINVAL, "null bank");
     cudaStream_t st = (cudaStream_t)stream;
-    CU_TRY(cudaSetDevice(bk->device));
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
     if (bk->free_pending[0] || bk->free_pending[1]) {      // chunks of the asynchronous host entry may still be in flight
         int rc = spiir_bank_host_sync(bk);
+        if (rc) return rc;
+    }
+    {
+        int rc = order_after_previous(bk, st);
         if (rc) return rc;
     }
     CU_TRY(cudaMemsetAsync(bk->y, 0, (size_t)std::max<int64_t>(bk->n_slots, 1) * 2 * sizeof(float), st));
     bk->pos = round_up(bk->D, 4);
     CU_TRY(cudaMemsetAsync(bk->tape[bk->cur], 0, (size_t)(bk->pos + 8) * sizeof(float), st));
-    if (bk->hstream) {      // the host-buffer entry works on the bank's own stream: order it behind this reset
-        CU_TRY(cudaEventRecord(bk->ev_reset, st));
-        CU_TRY(cudaStreamWaitEvent(bk->hstream, bk->ev_reset, 0));
-    }
     bk->poisoned = false;
     return SPIIR_OK;
 }
@@ -815,7 +897,12 @@ int spiir_bank_get_state(spiir_bank* bk, float* y_dev, float* hist_dev, void* st
 {
     if (!bk) return fail(SPIIR_EINVAL, "null bank");
     cudaStream_t st = (cudaStream_t)stream;
-    CU_TRY(cudaSetDevice(bk->device));
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
+    {
+        int rc = order_after_previous(bk, st);      // also behind chunks of the host-buffer entry that are still in flight
+        if (rc) return rc;
+    }
     if (y_dev) {
         const int threads = 256;
         spiir_permute_state_kernel<<<(unsigned)((bk->K + threads - 1) / threads), threads, 0, st>>>(
@@ -833,7 +920,12 @@ int spiir_bank_set_state(spiir_bank* bk, const float* y_dev, const float* hist_d
 {
     if (!bk) return fail(SPIIR_EINVAL, "null bank");
     cudaStream_t st = (cudaStream_t)stream;
-    CU_TRY(cudaSetDevice(bk->device));
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
+    {
+        int rc = order_after_previous(bk, st);
+        if (rc) return rc;
+    }
     if (y_dev) {
         const int threads = 256;
         spiir_permute_state_kernel<<<(unsigned)((bk->K + threads - 1) / threads), threads, 0, st>>>(
@@ -850,7 +942,7 @@ int spiir_bank_set_state(spiir_bank* bk, const float* y_dev, const float* hist_d
 int spiir_bank_destroy(spiir_bank* bk)
 {
     if (!bk) return SPIIR_OK;
-    cudaSetDevice(bk->device);
+    DeviceGuard dg(bk->device);
     cudaDeviceSynchronize();
     free_bank(bk);
     return SPIIR_OK;

@@ -58,6 +58,43 @@ def test_argument_validation_happens_before_any_device_work(pkg):
     assert lib.spiir_filter(None, None, 0, None, 0, None) == -1
 
 
+def test_every_invalid_blocking_pair_is_rejected_at_create(pkg):
+    # spiir.h lists the valid (filters_per_thread, warps_per_cta) pairs as a create-time contract: every other pair must
+    # come back SPIIR_EINVAL from spiir_bank_create itself (before any device work), not from the first spiir_filter
+    off = np.array([0, 300], np.int64)
+    rng = np.random.default_rng(3)
+    a1 = (0.9 * np.exp(1j * rng.uniform(0, 1, 300))).astype(np.complex64)
+    b0 = np.ones(300, np.complex64)
+    d = rng.integers(0, 50, 300).astype(np.int32)
+    valid = {(16, 8), (8, 8), (8, 16), (4, 8), (4, 16), (4, 32), (2, 32), (1, 32)}
+    import torch
+    for F in (1, 2, 4, 8, 16):
+        for W in (8, 16, 32):
+            opt = pkg.SpiirOptions(filters_per_thread=F, warps_per_cta=W)
+            if (F, W) in valid:
+                if torch.cuda.is_available():
+                    pkg.spiir_bank_destroy(pkg.spiir_bank_create(off, a1, b0, d, options=opt))
+                else:
+                    with pytest.raises(pkg.SpiirError) as ei:
+                        pkg.spiir_bank_create(off, a1, b0, d, options=opt)
+                    assert ei.value.code == -3                     # got past the validation, stopped at "no device"
+            else:
+                with pytest.raises(pkg.SpiirError) as ei:
+                    pkg.spiir_bank_create(off, a1, b0, d, options=opt)
+                assert ei.value.code == -1 and "unsupported blocking" in str(ei.value), (F, W)
+    # the streaming path comes with 8 warps: filters_per_thread 1 and 2 have no kernel there
+    for F in (1, 2):
+        with pytest.raises(pkg.SpiirError) as ei:
+            pkg.spiir_bank_create(off, a1, b0, d, options=pkg.SpiirOptions(path=pkg.PATH_STREAM, filters_per_thread=F))
+        assert ei.value.code == -1
+    # reserved must be 0
+    opt = pkg.SpiirOptions()
+    opt.reserved[0] = 7
+    with pytest.raises(pkg.SpiirError) as ei:
+        pkg.spiir_bank_create(off, a1, b0, d, options=opt)
+    assert ei.value.code == -1 and "reserved" in str(ei.value)
+
+
 def test_fails_loudly_without_a_gpu(pkg):
     import torch
     if torch.cuda.is_available():

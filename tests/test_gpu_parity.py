@@ -15,6 +15,7 @@ import spiir_inputs
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-4   # north_star tolerance, relative to the template's max |SNR_ref|
+PEAK_TOL = 2.01e-4   # what TOL implies for |SNR|^2 relative to max|SNR_ref|^2 (derivation at its use and in DESIGN.md section 5)
 
 
 @pytest.fixture(scope="module")
@@ -31,8 +32,9 @@ def env():
     return pkg, oracle, torch
 
 
-def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=False, small=0):
-    """Filter inp.x through a fresh bank in the given chunking; returns complex64 [T or len(rows), N]."""
+def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=False, small=0, device_result=False):
+    """Filter inp.x through a fresh bank in the given chunking; returns complex64 [T or len(rows), N]
+    (numpy, or the CUDA tensor itself with device_result)."""
     pkg, _, torch = env
     N = inp.n_samples
     chunks = [N] if chunks is None else list(chunks)
@@ -56,6 +58,8 @@ def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=Fals
                 pkg.spiir_filter(bank.handle, x[pos:pos], snr[:, pos:pos], ld=N, n=0)
             pos += c
         torch.cuda.synchronize()
+        if device_result:
+            return snr
         sel = snr if rows is None else snr[torch.as_tensor(np.asarray(rows), device="cuda")]
         return sel.cpu().numpy()
 
@@ -208,13 +212,16 @@ def test_window_split_over_several_launches(env):
     check(run_gpu(env, inp, path=2), ref)
 
 
-# ------------------------------------------------------------------ config 2 (chirp structure), streaming, sampled templates
-def test_cfg2_streaming_subset(env):
+# ------------------------------------------------------------------ config 2 (chirp structure), streaming, ALL templates
+def test_cfg2_streaming_full_bank(env):
+    # SURVEY.md section 8(c) GPU acceptance: the oracle on all templates for cfg0-cfg2 (3.4e10 filter-samples)
     inp = spiir_inputs.make_config(2)
-    rows = spiir_inputs.parity_subset(inp.n_templates, 24, 2)
-    ref = env[1].run_inputs(inp.select_templates(rows))
-    got = run_gpu(env, inp, chunks=[4096] * 16, rows=rows)
-    check(got, ref)
+    got = run_gpu(env, inp, chunks=[4096] * 16)
+    worst = 0.0
+    for r0 in range(0, inp.n_templates, 256):             # 256 templates at a time bounds the complex128 reference
+        rows = np.arange(r0, min(r0 + 256, inp.n_templates))
+        worst = max(worst, check(got[rows], env[1].run_inputs(inp.select_templates(rows))))
+    print(f"cfg2 full bank: max relative error {worst:.3e}")
 
 
 # ------------------------------------------------------------------ config 3 (headline) at full size, launch config of bench.py
@@ -222,7 +229,7 @@ def test_cfg3_full_size_subset_and_invariants(env):
     pkg, oracle, torch = env
     inp = spiir_inputs.make_config(3)
     T = inp.n_templates
-    rows = spiir_inputs.parity_subset(T, 16, 3)
+    rows = spiir_inputs.parity_subset(T, 128, 3)          # first, last and 126 random templates
     # plant copies of checked templates at other positions: must come out bitwise equal to their originals
     src = rows[:3]
     dst = np.array([17, 2048, T - 2])
@@ -252,14 +259,64 @@ def test_cfg4_tiny_chunks(env, path):
 
 
 def test_cfg4_full_bank_in_bench_configuration(env):
-    # the whole 8192-template bank (4.7 M filters), streaming blocking and 16-sample calls exactly as bench.py --config 4
-    # runs it; 64 calls, sampled templates stratified over the filter count
-    inp = spiir_inputs.make_config(4, n_samples=1024)
-    kt = np.diff(inp.offsets)
-    rows = np.sort(np.argsort(kt)[np.linspace(0, inp.n_templates - 1, 12).astype(int)])
-    ref = env[1].run_inputs(inp.select_templates(rows))
-    got = run_gpu(env, inp, chunks=[16] * 64, path=3, rows=rows)
+    # the whole 8192-template bank (4.7 M filters), streaming blocking and ALL 4096 calls of 16 samples exactly as
+    # bench.py --config 4 runs it: 128 templates stratified over the filter count against the
+    # oracle; the rest of the bank through the oracle-free invariants: planted duplicates and a template permutation
+    # must come out bitwise equal.  The 65 536 samples cross the tape's compaction point on path 3.
+    pkg, oracle, torch = env
+    inp0 = spiir_inputs.make_config(4)
+    T = inp0.n_templates
+    kt = np.diff(inp0.offsets)
+    rows = np.sort(np.argsort(kt, kind="stable")[np.linspace(0, T - 1, 128).astype(int)])
+    src = rows[[3, 40, 90, 127]]
+    dst = np.array([11, 4097, 6000, T - 3])
+    assert not np.intersect1d(dst, rows).size
+    idx = np.arange(T)
+    idx[dst] = src                                            # planted copies of checked templates
+    inp = inp0.select_templates(idx)
+    chunks = [16] * (inp.n_samples // 16)
+    a = run_gpu(env, inp, chunks=chunks, path=3, device_result=True)
+    assert torch.isfinite(torch.view_as_real(a)).all()
+    sel = a[torch.as_tensor(rows, device="cuda")].cpu().numpy()
+    err = check(sel, oracle.run_inputs(inp.select_templates(rows)))
+    print(f"cfg4 full bank, 4096 calls: max relative error {err:.3e} over {len(rows)} templates")
+    for s_, d_ in zip(src, dst):
+        assert torch.equal(torch.view_as_real(a[int(s_)]), torch.view_as_real(a[int(d_)]))
+    perm = np.random.default_rng(44).permutation(T)
+    b = run_gpu(env, inp.select_templates(perm), chunks=chunks, path=3, device_result=True)
+    assert torch.equal(torch.view_as_real(b), torch.view_as_real(a[torch.as_tensor(perm, device="cuda")]))
+
+
+@pytest.mark.parametrize("ragged", [False, True])
+def test_stream_path_across_tape_compaction(env, ragged):
+    # path 3 in its steady state: more than 2 x 65 536 samples in tiny calls without a reset, so the input tape is
+    # compacted (history moved to the other buffer) twice while the programmatic launch chain keeps running; with
+    # ragged calls the streaming kernels and the blocked fallback (n > 64) alternate across the compaction
+    pkg, oracle, torch = env
+    n = 2 * 65536 + 9000
+    inp = spiir_inputs.make_random_bank(71, [256, 100, 512, 64, 1024, 77, 300, 128] * 3, n, d_max=700)
+    ref = oracle.run_inputs(inp)
+    if ragged:
+        pat, chunks, left = [1, 7, 16, 64, 65], [], n
+        while left > 0:
+            c = min(left, pat[len(chunks) % len(pat)])
+            chunks.append(c)
+            left -= c
+    else:
+        chunks = [16] * (n // 16) + ([n % 16] if n % 16 else [])
+    got = run_gpu(env, inp, chunks=chunks, path=3)
     check(got, ref)
+    # the same stream through the blocked kernel in long calls: equal within tolerance (another summation tree)
+    one = run_gpu(env, inp, chunks=[65536, 65536, 9000], path=1)
+    assert rel_err(got, one.astype(np.complex128)).max() <= TOL
+
+
+def test_tape_grows_with_live_history(env):
+    # a small call, then one longer than the tape (65 536 + D): the tape is reallocated and must keep the history
+    inp = spiir_inputs.make_random_bank(72, [256, 90], 100 + 70000 + 50, d_max=3000)
+    ref = env[1].run_inputs(inp)
+    for path in (1, 2):
+        check(run_gpu(env, inp, chunks=[100, 70000, 50], path=path), ref)
 
 
 def test_mixed_template_sizes_over_many_cta_items(env):
@@ -338,6 +395,74 @@ def test_checkpoint_resume(env):
     assert np.array_equal(snr.cpu().numpy().view(np.float32), full.view(np.float32))
 
 
+def test_checkpoint_resume_through_the_host_entry_and_mixed_entries(env):
+    # set_state / spiir_filter on the caller's stream followed by the host-buffer entry (which runs on the bank's own
+    # streams), and get_state right after an asynchronous host call: the bank orders them itself (spiir.h)
+    pkg, _, torch = env
+    inp = spiir_inputs.make_random_bank(32, [300, 77, 512], 3000, d_max=500)
+    x = torch.from_numpy(inp.x).cuda()
+    xh = torch.from_numpy(inp.x).pin_memory()
+    opt = pkg.SpiirOptions(path=1)
+    T, N = inp.n_templates, inp.n_samples
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank:
+        full = np.empty((T, N), np.complex64)
+        for c0, c1 in ((0, 1000), (1000, 2200), (2200, 3000)):
+            pkg.spiir_filter_host(bank.handle, inp.x[c0:c1], full[:, c0:c1])
+    for _ in range(3):                                             # a race would not show every time
+        out = torch.empty((T, N), dtype=torch.complex64).pin_memory()
+        side = torch.cuda.Stream()
+        with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank:
+            pkg.spiir_filter_host_async(bank.handle, xh.numpy()[:1000], out.numpy()[:, :1000])
+            y = torch.empty(inp.n_filters, dtype=torch.complex64, device="cuda")
+            hist = torch.empty(bank.max_delay, dtype=torch.float32, device="cuda")
+            pkg.spiir_bank_get_state(bank.handle, y, hist, stream=side)          # no host sync in between
+            side.synchronize()
+            pkg.spiir_bank_host_sync(bank.handle)
+        with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank2:
+            pkg.spiir_bank_set_state(bank2.handle, y, hist, stream=side)         # caller's stream ...
+            pkg.spiir_filter_host_async(bank2.handle, xh.numpy()[1000:2200], out.numpy()[:, 1000:2200])   # ... bank's stream
+            dev = torch.empty((T, 800), dtype=torch.complex64, device="cuda")
+            pkg.spiir_filter(bank2.handle, x[2200:], dev, stream=side)           # and back to the caller's
+            side.synchronize()
+            pkg.spiir_bank_host_sync(bank2.handle)
+        got = out.numpy().copy()
+        got[:, 2200:] = dev.cpu().numpy()
+        assert np.array_equal(got.view(np.float32), full.view(np.float32))
+
+
+def test_calls_alternating_between_streams_are_ordered(env):
+    pkg, _, torch = env
+    inp = spiir_inputs.make_random_bank(33, [256, 256, 100, 700], 16 * 600, d_max=900)
+    ref = run_gpu(env, inp, chunks=[600] * 16, path=1)
+    x = torch.from_numpy(inp.x).cuda()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.current_stream()]
+    torch.cuda.synchronize()
+    for _ in range(3):
+        snr = torch.full((inp.n_templates, inp.n_samples), float("nan"), dtype=torch.complex64, device="cuda")
+        torch.cuda.synchronize()
+        with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, pkg.SpiirOptions(path=1)) as bank:
+            for i in range(16):
+                pkg.spiir_filter(bank.handle, x[600 * i:600 * (i + 1)], snr[:, 600 * i:600 * (i + 1)], stream=streams[i % 3])
+            torch.cuda.synchronize()
+        assert np.array_equal(snr.cpu().numpy().view(np.float32), ref.view(np.float32))
+
+
+def test_binding_rejects_mismatched_tensors(env):
+    pkg, _, torch = env
+    inp = spiir_inputs.make_random_bank(34, [64, 64, 64], 100, d_max=10)
+    x = torch.from_numpy(inp.x).cuda()
+    with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays) as bank:
+        with pytest.raises(ValueError):
+            pkg.spiir_filter(bank.handle, x, torch.empty((2, 100), dtype=torch.complex64, device="cuda"))      # too few rows
+        with pytest.raises(ValueError):
+            pkg.spiir_filter_peaks(bank.handle, x, torch.empty(2, dtype=torch.float32, device="cuda"),
+                                   torch.empty(3, dtype=torch.int32, device="cuda"))
+        with pytest.raises(ValueError):
+            pkg.spiir_filter_host_async(bank.handle, inp.x.astype(np.float64), np.empty((3, 100), np.complex64))   # would need a copy
+        with pytest.raises(ValueError):
+            pkg.spiir_filter_host_async(bank.handle, inp.x[::2], np.empty((3, 50), np.complex64))                 # strided
+
+
 def test_async_host_entry_back_to_back(env):
     pkg, oracle, torch = env
     inp = spiir_inputs.make_random_bank(43, [128, 512, 70], 3 * 8192 + 100, d_max=900)
@@ -388,9 +513,11 @@ def check_peaks(pkg, torch, oracle, inp, chunks, opt, with_snr, ref):
             p, i = power.cpu().numpy().astype(np.float64), index.cpu().numpy().astype(np.int64)
             scale = (np.abs(ref).max(axis=1)) ** 2
             assert np.all((i >= 0) & (i < c))
-            assert np.all(np.abs(p - p_ref) <= 4e-4 * scale), (np.abs(p - p_ref) / scale).max()
+            # |z|^2 with |z - z_ref| <= 1e-4 m, m = max|z_ref|: | |z|^2 - |z_ref|^2 | <= (2 |z_ref| + 1e-4 m) 1e-4 m
+            # <= 2.0001e-4 m^2; the FP32 evaluation of re^2 + im^2 adds < 2e-7 m^2
+            assert np.all(np.abs(p - p_ref) <= PEAK_TOL * scale), (np.abs(p - p_ref) / scale).max()
             at = np.abs(ref[np.arange(T), pos + i]) ** 2
-            assert np.all(p_ref - at <= 4e-4 * scale)
+            assert np.all(p_ref - at <= 2 * PEAK_TOL * scale)      # both the winner and the true maximum may move by PEAK_TOL
             if with_snr:
                 got = snr.cpu().numpy()
                 assert np.isfinite(got.view(np.float32)).all()
@@ -470,9 +597,13 @@ def test_fuzz_shapes_paths_blockings(env, seed):
     path = int(rng.integers(0, 4))
     F = int(rng.choice([0, 0, 1, 2, 4, 8, 16]))
     small = int(rng.integers(0, 3))
-    if path == 3 and F not in (0, 4, 8):
-        F = 0
     if small == 1 and F not in (0, 8):
+        F = 0
+    if path == 3 and F in (1, 2):
+        # no streaming blocking with 1 or 2 filters per thread: rejected at create (spiir.h), not at the first call
+        with pytest.raises(pkg.SpiirError) as ei:
+            run_gpu(env, inp, chunks=chunks, path=path, F=F, small=small)
+        assert ei.value.code == -1
         F = 0
     got = run_gpu(env, inp, chunks=chunks, path=path, F=F, small=small)
     err = check(got, ref)

@@ -1,5 +1,8 @@
-"""Multi-GPU host logic on CPU: templates shard across ranks with no
-data-path collective; the only exchange is the max-over-ranks of the timing.  world_size 2, gloo."""
+"""Multi-GPU HOST LOGIC only, on CPU: templates shard across ranks with no
+data-path collective; the only exchange is the max-over-ranks of the timing.  world_size 2, gloo.  No device call is
+made here (the oracle stands in for it so that the partition and the gather can be checked without a GPU); the device
+path of the same split -- two ranks filtering their shards through spiir_filter, gathered rows against the oracle and
+bitwise against the single-bank run -- is tests/test_sharding_gpu.py (-m gpu)."""
 import os
 import socket
 
