@@ -17,11 +17,11 @@ def parse(stdout):
     return json.loads(lines[0])
 
 
-def check_line(d, n_gpus=1):
+def check_line(d, n_gpus=1, scaling="weak"):
     for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
                 "vs_baseline", "dtype", "data", "config", "gpu_launches", "roofline", "clocks", "e2e"):
         assert key in d, key
-    assert d["n_gpus"] == n_gpus and d["value"] > 0 and d["dtype"] == "f32" and d["scaling"] == "weak"
+    assert d["n_gpus"] == n_gpus and d["value"] > 0 and d["dtype"] == "f32" and d["scaling"] == scaling
     assert d["gpu_launches"] > 0 and d["warmup"] >= 3 and d["vs_baseline"] is None
     r = d["roofline"]
     assert r["bound"] in ("alu", "hbm") and r["achieved"] > 0 and r["peak"] > 0 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
@@ -60,3 +60,34 @@ def test_bench_two_ranks_functional():
     assert r.returncode == 0, r.stderr[-2000:]
     d = parse(r.stdout)                     # exactly one line: only rank 0 prints
     check_line(d, n_gpus=2)
+    assert d.get("functional_only") is True           # two ranks on one GPU: marked, not a multi-GPU number
+
+
+def test_bench_two_ranks_shard_one_bank():
+    """--shard: ONE bank split over the ranks by shard_templates ("scaling": "strong"), per-rank filter counts in the line."""
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29735", str(ROOT / "bench.py"), "--gpus", "2",
+                        "--config", "1", "--steps", "1", "--warmup", "3", "--no-cpu-baseline", "--shard"],
+                       capture_output=True, text=True, cwd=ROOT, timeout=240,
+                       env=dict(os.environ, GLOO_SOCKET_IFNAME="lo", SPIIR_BENCH_BACKEND="gloo"))
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = parse(r.stdout)
+    check_line(d, n_gpus=2, scaling="strong")
+    sh = d["shard"]
+    assert sum(sh["filters_per_rank"]) == 64 * 256 and sh["imbalance_max_over_mean"] < 1.01
+
+
+def test_bench_default_run_reports_every_config():
+    """The driver's command: cfg3 as the headline plus a per_config leg for cfg0, cfg1 (one-shot and chunked), cfg2, cfg4."""
+    r = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--steps", "1", "--warmup", "3", "--cpu-templates", "4"],
+                       capture_output=True, text=True, cwd=ROOT, timeout=1500)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = parse(r.stdout)
+    check_line(d)
+    assert d["e2e"].get("last_chunk_bitwise_equal_to_device_run") is True
+    per = d["per_config"]
+    assert set(per) == {"cfg0", "cfg1_oneshot", "cfg1_chunked", "cfg2", "cfg4"}
+    for name, leg in per.items():
+        assert leg["value"] > 0 and leg["bound"] in ("alu", "hbm") and 0 < leg["frac"] < 1.2, name
+        assert leg["p50_us"] > 0 and leg["p99_us"] >= leg["p50_us"] and "reasons" in leg["clocks"], name
+    assert per["cfg4"]["bound"] == "hbm" and per["cfg4"]["path"] == 3 and per["cfg0"]["path"] == 2
