@@ -176,6 +176,53 @@ __device__ __forceinline__ void mbar_wait(u64* bar, unsigned parity)
         "DONE_%=:\n}" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
 }
 
+// Window staging (north_star subsystem (3): "stages the delayed input window into shared
+// memory with TMA or cp.async.bulk"; the paper's counterpart is the shared read-only-cache window).
+// One thread hands copy 0 of the window to the bulk-copy engine: cp.async.bulk global -> shared, completion counted in
+// bytes on an mbarrier (SASS: UBLKCP + SYNCS); the warps meanwhile fetch their coefficients.  Source and destination
+// are 16-byte aligned and the size a multiple of 16.  The NC - 1 shifted copies (copy c holds win[i + c]: a 4-byte
+// misalignment no bulk copy can produce) are then made shared -> shared by all threads.
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, u64* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_addr(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_addr(bar))
+                 : "memory");
+}
+// Called by ONE thread: arm the barrier for `bytes` and issue the copies (pieces of <= 32 KB).
+__device__ __forceinline__ void stage_window_issue(float* dst, const float* src, unsigned bytes, u64* bar)
+{
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");     // the init is visible to the copy engine
+    mbar_expect_tx(bar, bytes);
+    constexpr unsigned kPiece = 32768;
+    for (unsigned off = 0; off < bytes; off += kPiece)
+        bulk_copy_g2s(reinterpret_cast<char*>(dst) + off, reinterpret_cast<const char*>(src) + off,
+                      bytes - off < kPiece ? bytes - off : kPiece, bar);
+}
+// All threads, once copy 0 is complete in shared memory (and visible: a __syncthreads or the copy's mbarrier): build the
+// NC - 1 shifted copies from it (float4 i of copy 0 -> 4 scalar stores per further copy).
+template <int NC>
+__device__ __forceinline__ void make_shifted_copies(float* smem, int64_t cstride, int tid, int n_threads)
+{
+    if (NC == 1) return;
+    const int n4 = (int)(cstride / 4);
+    for (int i = tid; i < n4; i += n_threads) {
+        const float4 v = reinterpret_cast<const float4*>(smem)[i];
+        const float e[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int c = 1; c < NC; ++c) {
+            float* dst = smem + (int64_t)c * cstride + 4 * i - c;
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (4 * i + q - c >= 0) dst[q] = e[q];
+        }
+    }
+}
+
 // Sum the partial rows of the warps of one template for ns samples and store them (fixed order over warps).
 // The ns samples are shared out over the lanes of the template's warps.
 // |z|^2 and the sample index packed so that an unsigned max picks the largest power and, among equals, the earliest
@@ -289,7 +336,7 @@ __device__ __forceinline__ void seg_reduce_store(u64 (&S)[kTT], u64* __restrict_
 
 // Shared memory of the filter kernel, in this order:
 //   NC window copies of `cstride` floats each (absent when GMEM_X), W transpose scratches, kPB x W x kTS partial sums,
-//   W x kPB mbarriers
+//   W x kPB mbarriers of the template hand-over + 1 mbarrier of the window's bulk copy
 __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_len, bool gmem_x, int64_t* cstride_out,
                                                      int part_buffers = kPB)
 {
@@ -297,7 +344,7 @@ __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_l
     const int64_t cstride = gmem_x ? 0 : ((win_len + 16 + 31) / 32 * 32);
     if (cstride_out) *cstride_out = cstride;
     return (size_t)(gmem_x ? 0 : NC * cstride) * sizeof(float) + (size_t)W * kTrWarp * sizeof(u64) +
-           (size_t)part_buffers * W * super_tile(W) * sizeof(u64) + (size_t)W * kPB * sizeof(u64);
+           (size_t)part_buffers * W * super_tile(W) * sizeof(u64) + (size_t)(W * kPB + 1) * sizeof(u64);
 }
 
 // Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
@@ -319,37 +366,19 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     const int64_t nseg = min(p.seg_len, p.n - t0);
     if (nseg <= 0) return;
 
-    // ---- stage the input window [t0 - w0, t0 + nseg) into shared memory, NC times (copy c shifted by c)
+    // ---- stage the input window [t0 - w0, t0 + nseg) into shared memory, NC times (copy c shifted by c): copy 0 by
+    // one bulk copy (cp.async.bulk + mbarrier complete_tx), the shifted copies shared -> shared
     const int win_len = p.w0 + (int)nseg;
     int64_t cstride;
     filter_smem_bytes(W, NC, win_len, GMEM_X, &cstride);
-    const float* xs;
-    if (GMEM_X) {
-        xs = p.xwin + t0;
-    } else {
-        const float4* src = reinterpret_cast<const float4*>(p.xwin + t0);   // t0 and xwin are 16-byte aligned
-        const int n4 = (int)(cstride / 4);
-        const int v4 = (win_len + 3) / 4;                                    // float4s that hold valid samples
-        for (int i = tid; i < n4; i += kThreads) {
-            const float4 v = i < v4 ? src[i] : make_float4(0.f, 0.f, 0.f, 0.f);
-            reinterpret_cast<float4*>(smem)[i] = v;
-            if (NC > 1) {
-                const float e[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                for (int c = 1; c < NC; ++c) {
-                    float* dst = smem + (int64_t)c * cstride + 4 * i - c;
-#pragma unroll
-                    for (int q = 0; q < 4; ++q)
-                        if (4 * i + q - c >= 0) dst[q] = e[q];
-                }
-            }
-        }
-        xs = smem;
-    }
     u64* trbuf = reinterpret_cast<u64*>(smem + (GMEM_X ? 0 : NC * cstride));   // [W][kTrWarp]
     u64* part64 = trbuf + (size_t)W * kTrWarp;                                 // [kPB][W][TS]
-    u64* bars = part64 + (size_t)(kAsync ? kPB : 2) * W * TS;                                // [W][kPB], indexed by a group's first warp
+    u64* bars = part64 + (size_t)(kAsync ? kPB : 2) * W * TS;                  // [W][kPB], indexed by a group's first warp
+    u64* stage_bar = bars + (size_t)W * kPB;
     u64* mytr = trbuf + (size_t)warp * kTrWarp;
+    const float* xs = GMEM_X ? p.xwin + t0 : smem;
+    const int staged = (win_len + 3) / 4 * 4;                                  // floats the bulk copy brings (16-byte units)
+    if (!GMEM_X && tid == 0) stage_window_issue(smem, p.xwin + t0, (unsigned)staged * 4u, stage_bar);   // t0, xwin: 16-byte aligned
     // per-template hand-over without any CTA-wide barrier: only where one CTA owns the SM and all rounds have one shape
     const bool sums = PEAK ? (p.snr || p.peaks) : (p.snr != nullptr);                                        // false: carry pass, states only
     const bool async = kAsync && p.uniform_groups && sums;
@@ -359,7 +388,15 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
             for (int b = 0; b < kPB; ++b) mbar_init(bars + tid * kPB + b, count);
     }
     unsigned use = 0;                                                          // super tiles this warp has produced
-    __syncthreads();
+    __syncthreads();                                                           // barrier inits visible to every thread
+    if (!GMEM_X) {
+        mbar_wait(stage_bar, 0);                                               // copy 0 has landed
+        // zero what lies behind the valid samples (partial register tiles read a few floats beyond them)
+        for (int k = win_len + tid; k < (int)cstride; k += kThreads) smem[k] = 0.f;
+        if (NC > 1) __syncthreads();
+        make_shifted_copies<NC>(smem, cstride, tid, kThreads);
+        __syncthreads();
+    }
 
     const bool last_seg = (t0 + nseg >= p.n);
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
@@ -494,7 +531,8 @@ __host__ __device__ inline size_t stream_smem_bytes(int F, int NC, int64_t win_l
 {
     const int64_t cstride = (win_len + 16 + 31) / 32 * 32;
     if (cstride_out) *cstride_out = cstride;
-    return (size_t)(NC * cstride) * sizeof(float) + (size_t)stream_warps(F) * kTrWarp * sizeof(u64);
+    // window copies, one transpose scratch per warp, the mbarrier of the window's bulk copy
+    return (size_t)(NC * cstride) * sizeof(float) + (size_t)stream_warps(F) * kTrWarp * sizeof(u64) + 2 * sizeof(u64);
 }
 
 // The 7F cache lines of a warp tile's coefficients and state, one or two per lane, requested into L1.
@@ -521,42 +559,28 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
     const int win_len = p.w0 + p.n;
     int64_t cstride;
     stream_smem_bytes(F, NC, win_len, &cstride);
+    u64* const stage_bar = reinterpret_cast<u64*>(smem + NC * cstride) + (size_t)kStreamWarps * kTrWarp;   // completion of the window's bulk copy
     // the first tile's coefficients travel while the window is staged
     if ((int64_t)blockIdx.x * kStreamWarps + warp < p.n_tiles) stream_prefetch_tile<F>(p, (int64_t)blockIdx.x * kStreamWarps + warp, lane);
     // Launched with programmatic dependent launch: the grid is set up and the first coefficients are requested while the
-    // previous kernel in the stream (normally the previous call's combine pass) is still running.  Everything read from
-    // here on may have been written by that kernel's predecessors or by the caller's own kernels: wait for them.
+    // previous kernel in the stream (normally the previous call) is still running.  Everything read from here on may
+    // have been written by that kernel or by the caller's own kernels: wait for them.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     {
-        const float4* src = reinterpret_cast<const float4*>(p.xwin);
-        const int n4 = (int)(cstride / 4), v4 = (win_len + 3) / 4;
-        for (int i = tid; i < n4; i += kThreads) {
-            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (i < v4) {
-                if (!p.xnew || 4 * i + 3 < p.w0) {
-                    v = src[i];
-                } else {                               // the float4 that straddles history and chunk, and the chunk itself
-                    float e[4];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const int k = 4 * i + q;
-                        e[q] = k < p.w0 ? p.xwin[k] : (k < win_len ? p.xnew[k - p.w0] : 0.f);
-                    }
-                    v = make_float4(e[0], e[1], e[2], e[3]);
-                }
-            }
-            reinterpret_cast<float4*>(smem)[i] = v;
-            if (NC > 1) {
-                const float e[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                for (int c = 1; c < NC; ++c) {
-                    float* dst = smem + (int64_t)c * cstride + 4 * i - c;
-#pragma unroll
-                    for (int q = 0; q < 4; ++q)
-                        if (4 * i + q - c >= 0) dst[q] = e[q];
-                }
-            }
+        // copy 0 of the window: the part that is whole 16-byte units of the tape by one bulk copy (cp.async.bulk +
+        // mbarrier complete_tx); the few floats behind it (and the chunk itself while it is
+        // still in the caller's buffer) by ordinary loads; then the shifted copies shared -> shared
+        const int bulk_floats = p.xnew ? p.w0 / 4 * 4 : (win_len + 3) / 4 * 4;
+        if (tid == 0 && bulk_floats > 0) stage_window_issue(smem, p.xwin, (unsigned)bulk_floats * 4u, stage_bar);
+        for (int k = bulk_floats + tid; k < (int)cstride; k += kThreads)
+            smem[k] = k < p.w0 ? p.xwin[k] : (k < win_len ? p.xnew[k - p.w0] : 0.f);
+        __syncthreads();                               // the barrier's init and the stores above are visible
+        if (bulk_floats > 0) mbar_wait(stage_bar, 0);
+        if (bulk_floats > win_len) {                   // the copy brought up to 3 floats from beyond the window
+            if (win_len + tid < bulk_floats) smem[win_len + tid] = 0.f;
+            __syncthreads();
         }
+        make_shifted_copies<NC>(smem, cstride, tid, kThreads);
     }
     const float* xs = smem;
     u64* mytr = reinterpret_cast<u64*>(smem + NC * cstride) + (size_t)warp * kTrWarp;
