@@ -217,7 +217,8 @@ def measure(ctx, args, cfg, steps, warmup, *, chunk=None, e2e=False, label=None)
     if path == 0 and L <= 64 and inp.n_filters >= (1 << 20):
         path = pkg.PATH_STREAM            # tiny chunks over a large bank: the HBM-bound streaming blocking
     opt = pkg.SpiirOptions(path=path, filters_per_thread=args.filters_per_thread, warps_per_cta=args.warps_per_cta,
-                           window_copies=args.window_copies, scan_segments=args.scan_segments)
+                           window_copies=args.window_copies, scan_segments=args.scan_segments,
+                           scan_launches=args.scan_launches)
     bank = pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, dev_index, opt)
     x = torch.from_numpy(inp.x).cuda()
     keep_whole = (T * N * 8) <= args.max_snr_bytes
@@ -227,17 +228,21 @@ def measure(ctx, args, cfg, steps, warmup, *, chunk=None, e2e=False, label=None)
     peak_index = torch.empty(T, dtype=torch.int32, device="cuda")
     n_calls = (N + L - 1) // L
 
+    # the tensor views of every call are made once (slicing a tensor costs more host time than a cfg0 call takes on the GPU)
+    views = []
+    for c0 in range(0, N, L):
+        n = min(L, N - c0)
+        views.append((x[c0:c0 + n], snr[:, c0:c0 + n] if keep_whole else snr[:, :n]))
+
     def one_step(events=None):
         bank.reset()
-        for i, c0 in enumerate(range(0, N, L)):
+        for i, (xin, out) in enumerate(views):
             if events is not None:
                 events[i].record(stream)
-            n = min(L, N - c0)
-            out = snr[:, c0:c0 + n] if keep_whole else snr[:, :n]
             if args.peaks:
-                pkg.spiir_filter_peaks(bank.handle, x[c0:c0 + n], peak_power, peak_index, None if args.peaks == 1 else out)
+                pkg.spiir_filter_peaks(bank.handle, xin, peak_power, peak_index, None if args.peaks == 1 else out)
             else:
-                pkg.spiir_filter(bank.handle, x[c0:c0 + n], out)
+                pkg.spiir_filter(bank.handle, xin, out)
         if events is not None:
             events[n_calls].record(stream)
 
@@ -431,6 +436,7 @@ def main():
     ap.add_argument("--warps-per-cta", type=int, default=0)
     ap.add_argument("--window-copies", type=int, default=0)
     ap.add_argument("--scan-segments", type=int, default=0)
+    ap.add_argument("--scan-launches", type=int, default=0, help="3: three-launch form of the time-parallel path")
     ap.add_argument("--peaks", type=int, default=0, help="1: spiir_filter_peaks without SNR output, 2: with (not the headline)")
     ap.add_argument("--max-snr-bytes", type=float, default=20e9, help="keep the whole [T][N] SNR if it fits")
     ap.add_argument("--e2e-steps", type=int, default=2)

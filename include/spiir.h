@@ -81,7 +81,9 @@ typedef struct spiir_options {
     int32_t small_templates;    /* templates of <= 128 filters sharing warp tiles (sub-warp segments):
                                    0 = choose, 1 = on (forces the (8,16) blocking), 2 = off.  Not used with
                                    SPIIR_PATH_STREAM. */
-    int32_t reserved[1];        /* must be 0 (checked) */
+    int32_t scan_launches;      /* SPIIR_PATH_SCAN: 0 = choose (one cooperative launch per call when every CTA of the
+                                   items x segments grid is resident, else three), 3 = always the three-launch form
+                                   (carry pass, carry scan, output pass); any other value is SPIIR_EINVAL */
 } spiir_options;
 
 /* Build a bank.  All pointers are HOST pointers; the arrays are copied, the caller keeps ownership.

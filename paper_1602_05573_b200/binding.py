@@ -29,16 +29,17 @@ class SpiirOptions(ctypes.Structure):
     _fields_ = [("struct_size", ctypes.c_int32), ("path", ctypes.c_int32),
                 ("filters_per_thread", ctypes.c_int32), ("scan_segments", ctypes.c_int32),
                 ("warps_per_cta", ctypes.c_int32), ("window_copies", ctypes.c_int32),
-                ("small_templates", ctypes.c_int32), ("reserved", ctypes.c_int32 * 1)]
+                ("small_templates", ctypes.c_int32), ("scan_launches", ctypes.c_int32)]
 
     def __init__(self, path: int = PATH_AUTO, filters_per_thread: int = 0, scan_segments: int = 0,
-                 warps_per_cta: int = 0, window_copies: int = 0, small_templates: int = 0):
+                 warps_per_cta: int = 0, window_copies: int = 0, small_templates: int = 0, scan_launches: int = 0):
         super().__init__()
         self.struct_size = ctypes.sizeof(SpiirOptions)
         self.path, self.filters_per_thread, self.scan_segments = path, filters_per_thread, scan_segments
         self.warps_per_cta = warps_per_cta
         self.window_copies = window_copies
         self.small_templates = small_templates
+        self.scan_launches = scan_launches
 
 
 def library_path() -> Path:

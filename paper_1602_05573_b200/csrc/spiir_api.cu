@@ -101,6 +101,11 @@ struct spiir_bank {
     // scan scratch
     float *zbuf = nullptr, *cbuf = nullptr;
     int64_t scan_cap_seg = 0;
+    unsigned long long* scan_barrier = nullptr;   // arrival counter of the single-launch scan kernel (monotonic)
+    unsigned long long scan_arrivals = 0;         // its value once every launch enqueued so far has completed
+    bool scan_fused_configured = false;
+    int scan_fused_occ = -1;
+    size_t scan_fused_occ_smem = 0;
     // host-path scratch
     float* hx = nullptr;
     float* hsnr[2] = {nullptr, nullptr};
@@ -135,7 +140,7 @@ void free_bank(spiir_bank* bk)
     if (!bk) return;
     cudaFree(bk->coef); cudaFree(bk->y);
     cudaFree(bk->item_round0); cudaFree(bk->canon); cudaFree(bk->tile_begin); cudaFree(bk->stream_scratch); cudaFree(bk->peaks); cudaFree(bk->peak_snr); cudaFree(bk->work); cudaFree(bk->slot_of_filter);
-    cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf);
+    cudaFree(bk->tape[0]); cudaFree(bk->tape[1]); cudaFree(bk->zbuf); cudaFree(bk->cbuf); cudaFree(bk->scan_barrier);
     cudaFree(bk->hx); cudaFree(bk->hsnr[0]); cudaFree(bk->hsnr[1]);
     for (int i = 0; i < 2; ++i) {
         if (bk->ev_done[i]) cudaEventDestroy(bk->ev_done[i]);
@@ -244,6 +249,26 @@ const void* select_kernel(int F, int W, int NC, bool g, bool peak = false, bool 
 }
 
 bool valid_blocking(int F, int W) { return select_kernel(F, W, 1, false) != nullptr; }
+
+// Single-launch time-parallel kernel: the blockings that own an SM (one CTA per SM), shared-memory window, no trigger
+// reduction, no shared tiles (those take the three-launch form of the same path).
+const void* select_scan_fused_kernel(int F, int W, int NC)
+{
+#define SPIIR_FUSED(F_, W_)                                                                         \
+    if (F == F_ && W == W_) {                                                                        \
+        if (NC == 4) return (const void*)spiir_scan_fused_kernel<F_, W_, 4, false, false, false>;    \
+        if (NC == 2) return (const void*)spiir_scan_fused_kernel<F_, W_, 2, false, false, false>;    \
+        return (const void*)spiir_scan_fused_kernel<F_, W_, 1, false, false, false>;                 \
+    }
+    SPIIR_FUSED(16, 8)
+    SPIIR_FUSED(8, 16)
+    SPIIR_FUSED(4, 16)
+    SPIIR_FUSED(4, 32)
+    SPIIR_FUSED(2, 32)
+    SPIIR_FUSED(1, 32)
+#undef SPIIR_FUSED
+    return nullptr;
+}
 
 int default_warps(int F) { return F >= 16 ? 8 : (F == 8 ? 16 : 32); }
 
@@ -391,14 +416,23 @@ int run_stream(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr,
 }
 
 // Run the filter kernels over n samples whose window starts at xwin (aligned), sample 0 at xwin[w0].
-int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st, u64* peaks)
+// x_dev / append: the chunk is not on the tape yet; every path but the single-launch scan kernel (which reads the caller's
+// buffer and appends the chunk itself) first copies it there.
+int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, int64_t ld, cudaStream_t st, u64* peaks,
+              const float* x_dev, float* append)
 {
+    bool appended = false;
+    auto append_chunk = [&]() -> cudaError_t {
+        if (appended) return cudaSuccess;
+        appended = true;
+        return cudaMemcpyAsync(append, x_dev, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    };
     const size_t smem_cap = bk->smem_optin;
     // window floats per copy that fit beside the reduction buffers (a copy is padded by up to 47 floats)
     const int64_t max_win = ((int64_t)smem_cap - (int64_t)fixed_smem(bk->F, bk->W)) / (4 * bk->NC) - 48;
     const bool gmem = bk->gmem_only;          // history alone does not fit: read x through L1/L2
     int path = bk->opt.path;
-    if (stream_applies(bk, w0, n)) return run_stream(bk, xwin, w0, n, snr, ld, st, peaks);
+    if (stream_applies(bk, w0, n)) { CU_TRY(append_chunk()); return run_stream(bk, xwin, w0, n, snr, ld, st, peaks); }
     // ---- how much time-parallelism is needed to fill the machine?  The scan path does the recurrence twice, so it
     // only pays when the bank leaves at least half of the SMs idle (cfg2: 128 items on 148 SMs run 1.7x faster
     // sequentially).
@@ -412,6 +446,7 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     }
     if (n_seg <= 1) {
         // ------------------------------------------------ sequential-in-time path
+        CU_TRY(append_chunk());
         bk->last_path = SPIIR_PATH_THROUGHPUT;
         int64_t sub = n;
         if (!gmem) {
@@ -457,6 +492,50 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     if (rc) return rc;
     if (occ < 1) return fail(SPIIR_ECUDA, "filter kernel does not fit on an SM (smem %zu)", smem);
     const unsigned gx = (unsigned)bk->n_items;
+    // ---- one cooperative launch when every CTA of the (items x segments) grid is resident (cfg0, cfg1)
+    const void* fused = (n_seg > 1 && !gmem && !peaks && !bk->segmented && bk->opt.scan_launches != 3)
+                            ? select_scan_fused_kernel(bk->F, bk->W, bk->NC) : nullptr;
+    if (fused) {
+        if (!bk->scan_fused_configured) {
+            CU_TRY(cudaFuncSetAttribute(fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bk->smem_optin));
+            bk->scan_fused_configured = true;
+        }
+        if (bk->scan_fused_occ < 0 || bk->scan_fused_occ_smem != smem) {
+            int o = 0;
+            CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, fused, kWarp * bk->W, smem));
+            bk->scan_fused_occ = o;
+            bk->scan_fused_occ_smem = smem;
+        }
+        if ((int64_t)gx * n_seg > (int64_t)bk->n_sm * bk->scan_fused_occ) fused = nullptr;
+    }
+    if (fused) {
+        if (!bk->scan_barrier) {
+            CU_TRY(cudaMalloc((void**)&bk->scan_barrier, sizeof(unsigned long long)));
+            CU_TRY(cudaMemsetAsync(bk->scan_barrier, 0, sizeof(unsigned long long), st));
+            bk->scan_arrivals = 0;
+        }
+        ScanFusedParams sp{};
+        sp.pass1 = base_params(bk);
+        sp.pass1.y_in = nullptr; sp.pass1.y_out = bk->zbuf; sp.pass1.y_out_stride = 2 * bk->n_slots; sp.pass1.store_last_only = 0;
+        sp.pass1.xwin = xwin; sp.pass1.w0 = w0; sp.pass1.n = (n_seg - 1) * seg_len; sp.pass1.seg_len = seg_len;
+        sp.pass1.snr = nullptr; sp.pass1.ld = 0;
+        sp.pass2 = base_params(bk);
+        sp.pass2.y_in = bk->cbuf; sp.pass2.y_in_stride = 2 * bk->n_slots; sp.pass2.y_out = bk->y; sp.pass2.y_out_stride = 0;
+        sp.pass2.store_last_only = 1;
+        sp.pass2.xwin = xwin; sp.pass2.w0 = w0; sp.pass2.n = n; sp.pass2.seg_len = seg_len;
+        sp.pass2.snr = snr; sp.pass2.ld = ld;
+        sp.cbuf = bk->cbuf; sp.z = bk->zbuf; sp.y = bk->y; sp.n_slots = bk->n_slots; sp.n_seg = (int32_t)n_seg;
+        sp.xnew = x_dev; sp.append = append;
+        sp.barrier = bk->scan_barrier;
+        sp.target = bk->scan_arrivals + (unsigned long long)gx * (unsigned long long)n_seg;
+        bk->scan_arrivals += 2ull * gx * (unsigned long long)n_seg;      // two grid-wide barriers per launch
+        void* args[] = {(void*)&sp};
+        // cooperative launch: the driver checks that the whole grid is resident, which the two grid-wide barriers need
+        CU_TRY(cudaLaunchCooperativeKernel(fused, dim3(gx, (unsigned)n_seg, 1), dim3((unsigned)(kWarp * bk->W), 1, 1), args, smem, st));
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        return SPIIR_OK;
+    }
+    CU_TRY(append_chunk());
     if (n_seg > 1) {
         // pass 1: zero-state end values of segments 0 .. n_seg-2 (no sums, no output)
         FilterParams p = base_params(bk);
@@ -588,8 +667,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         if (o.window_copies != 0 && o.window_copies != 1 && o.window_copies != 2 && o.window_copies != 4)
             return fail(SPIIR_EINVAL, "window_copies must be 0, 1, 2 or 4");
         if (o.small_templates < 0 || o.small_templates > 2) return fail(SPIIR_EINVAL, "small_templates must be 0, 1 or 2");
-        if (opt->struct_size >= (int32_t)sizeof(spiir_options) && o.reserved[0] != 0)
-            return fail(SPIIR_EINVAL, "spiir_options.reserved must be 0");
+        if (o.scan_launches != 0 && o.scan_launches != 3) return fail(SPIIR_EINVAL, "scan_launches must be 0 or 3");
     }
     // ---- blocking: F filters per thread, W warps per CTA, shared tiles or not (host logic, no device needed)
     const bool stream = (o.path == SPIIR_PATH_STREAM);     // tiny chunks: small CTAs, several per SM
@@ -612,6 +690,13 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
         if (any_small && (o.small_templates == 1 || packed < plain_cost)) {
             F = 8; W = 16; segmented = true;
         }
+    }
+    // A bank that fits one CTA at one filter per lane (<= 32 warps x 32 lanes) is bound by latency, not by issue slots:
+    // one filter per thread (PAPER.md:L335 one warp per small template) spreads it over the most warps.
+    if (!stream && !segmented && !o.filters_per_thread && (o.warps_per_cta == 0 || o.warps_per_cta == 32)) {
+        int64_t slots1 = 0;
+        for (int32_t t = 0; t < T; ++t) slots1 += round_up(off[t + 1] - off[t], kWarp);
+        if (slots1 <= 32 * kWarp) { F = 1; W = 32; }
     }
     // The (filters_per_thread, warps_per_cta) pair must be one a compiled kernel serves: checked here, not at the first
     // spiir_filter.  When only one of the two was requested the other follows it.
@@ -733,8 +818,7 @@ int filter_impl(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, i
         // history + chunk itself and appends the chunk to the tape
         rc = run_stream(bk, tape + start_al, w0, n, snr_dev, ld, st, peaks, x_dev, tape + bk->pos);
     } else {
-        CU_TRY(cudaMemcpyAsync(tape + bk->pos, x_dev, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st));
-        rc = run_chunk(bk, tape + start_al, w0, n, snr_dev, ld, st, peaks);
+        rc = run_chunk(bk, tape + start_al, w0, n, snr_dev, ld, st, peaks, x_dev, tape + bk->pos);
     }
     if (rc) { bk->poisoned = true; return rc; }
     bk->pos += n;

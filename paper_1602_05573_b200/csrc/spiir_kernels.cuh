@@ -22,7 +22,8 @@
 //       time-parallel scan path, long calls of streaming banks); PEAK adds the fused trigger reduction, SEG the shared
 //       warp tiles of small templates
 //   spiir_stream_kernel<F, NC> + spiir_stream_combine_kernel   tiny chunks: independent warps + ordered combine
-//   spiir_scan_carry_kernel                                    carry combine of the scan path, in double
+//   spiir_scan_carry_kernel                                    carry combine of the scan path (powers from double)
+//   spiir_scan_fused_kernel<F, W, NC, ...>                     the scan path in one launch (two grid-wide barriers)
 //   spiir_unpack_peaks_kernel, spiir_permute_state_kernel      small utilities
 #pragma once
 #include <cuda_runtime.h>
@@ -347,13 +348,15 @@ __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_l
            (size_t)part_buffers * W * super_tile(W) * sizeof(u64) + (size_t)(W * kPB + 1) * sizeof(u64);
 }
 
-// Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
 // MINB = CTAs the register allocation must leave room for on one SM (tiny-chunk streaming: several small CTAs
 // per SM overlap one CTA's coefficient loads with another's arithmetic).
 // PEAK compiles the fused trigger reduction in (spiir_filter_peaks); the plain kernel is untouched by it.
 // SEG compiles the shared-tile path for banks of small templates in.
-template <int F, int W, int NC, bool GMEM_X, int MINB = 1, bool PEAK = false, bool SEG = false>
-__global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const FilterParams p)
+// The body of the blocked kernel for time segment `seg`, items item0, item0 + item_stride, ...; `staged` = the window of this
+// segment is already in shared memory (second pass of the fused time-parallel kernel).
+template <int F, int W, int NC, bool GMEM_X, int MINB, bool PEAK, bool SEG>
+__device__ __forceinline__ void filter_body(const FilterParams& p, const int seg, const int item0, const int item_stride,
+                                            const bool staged)
 {
     static_assert(!GMEM_X || NC == 1, "the global-memory window variant reads scalars");
     constexpr int kThreads = kWarp * W;
@@ -361,7 +364,6 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     constexpr int TS = super_tile(W);
     extern __shared__ __align__(16) float smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int seg = blockIdx.y;
     const int64_t t0 = (int64_t)seg * p.seg_len;             // first sample of this segment in the launch
     const int64_t nseg = min(p.seg_len, p.n - t0);
     if (nseg <= 0) return;
@@ -377,8 +379,8 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     u64* stage_bar = bars + (size_t)W * kPB;
     u64* mytr = trbuf + (size_t)warp * kTrWarp;
     const float* xs = GMEM_X ? p.xwin + t0 : smem;
-    const int staged = (win_len + 3) / 4 * 4;                                  // floats the bulk copy brings (16-byte units)
-    if (!GMEM_X && tid == 0) stage_window_issue(smem, p.xwin + t0, (unsigned)staged * 4u, stage_bar);   // t0, xwin: 16-byte aligned
+    const int staged_floats = (win_len + 3) / 4 * 4;                           // floats the bulk copy brings (16-byte units)
+    if (!GMEM_X && !staged && tid == 0) stage_window_issue(smem, p.xwin + t0, (unsigned)staged_floats * 4u, stage_bar);   // t0, xwin: 16-byte aligned
     // per-template hand-over without any CTA-wide barrier: only where one CTA owns the SM and all rounds have one shape
     const bool sums = PEAK ? (p.snr || p.peaks) : (p.snr != nullptr);                                        // false: carry pass, states only
     const bool async = kAsync && p.uniform_groups && sums;
@@ -389,7 +391,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     }
     unsigned use = 0;                                                          // super tiles this warp has produced
     __syncthreads();                                                           // barrier inits visible to every thread
-    if (!GMEM_X) {
+    if (!GMEM_X && !staged) {
         mbar_wait(stage_bar, 0);                                               // copy 0 has landed
         // zero what lies behind the valid samples (partial register tiles read a few floats beyond them)
         for (int k = win_len + tid; k < (int)cstride; k += kThreads) smem[k] = 0.f;
@@ -399,7 +401,7 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
     }
 
     const bool last_seg = (t0 + nseg >= p.n);
-    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+    for (int item = item0; item < p.n_items; item += item_stride) {
         const int r0 = p.item_round0[item], r1 = p.item_round0[item + 1];
         for (int r = r0; r < r1; ++r) {
             WarpWork ww = p.work[r * W + warp];
@@ -504,6 +506,135 @@ __global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const Fil
             if (sums && !async) __syncthreads();      // part rows are rewritten in the next round
         }
     }
+}
+
+// Main kernel.  grid.x strides over items, grid.y = time segments (1 for the sequential path).
+template <int F, int W, int NC, bool GMEM_X, int MINB = 1, bool PEAK = false, bool SEG = false>
+__global__ void __launch_bounds__(kWarp * W, MINB) spiir_filter_kernel(const FilterParams p)
+{
+    filter_body<F, W, NC, GMEM_X, MINB, PEAK, SEG>(p, (int)blockIdx.y, (int)blockIdx.x, (int)gridDim.x, false);
+}
+
+// ---- time-parallel path in ONE launch (north_star subsystem (4)).  Grid = items x segments,
+// every CTA resident (cooperative launch).  Phase 1: the segment from zero state, end states z_seg to global memory
+// (no sums); grid-wide barrier; the grid's threads then derive the true start states of all segments, one filter
+// slot per thread, c_{q+1} = a1^L c_q + z_q from c_0 = carried state (a1^L from double, SURVEY.md section 8(c) finding F2), with
+// the same arithmetic and rounding as spiir_scan_carry_kernel; a second barrier; every CTA runs its segment again with sums and
+// output.  The window stays
+// in shared memory between the phases.
+// c <- A c + z in FP32 (A = a1^L rounded from double); one fixed order of fused multiply-adds, shared by the standalone carry
+// kernel and the single-launch kernel so that both forms of the path produce the same bits
+__device__ __forceinline__ void scan_carry_step(float Ar, float Ai, float zr, float zi, float& cr, float& ci)
+{
+    const float nr = fmaf(Ar, cr, fmaf(-Ai, ci, zr));
+    const float ni = fmaf(Ar, ci, fmaf(Ai, cr, zi));
+    cr = nr; ci = ni;
+}
+
+struct ScanFusedParams {
+    FilterParams pass1, pass2;
+    float* cbuf;                     // [n_seg][2 n_slots] start states
+    const float* z;                  // = pass1.y_out
+    const float* y;                  // carried state (slot order)
+    int64_t n_slots;
+    int32_t n_seg;
+    const float* xnew;               // the call's chunk in the caller's buffer (not on the tape yet) ...
+    float* append;                   // ... and where it goes on the tape: every CTA appends its own segment
+    unsigned long long* barrier;     // monotonic arrival counter
+    unsigned long long target;       // its value when every CTA of this launch has arrived at the first barrier
+};
+
+__device__ __forceinline__ void grid_barrier(unsigned long long* counter, unsigned long long target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();                                                      // this CTA's end states are visible device-wide
+        atomicAdd(counter, 1ull);
+        unsigned long long v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(counter) : "memory");
+        } while (v < target);
+    }
+    __syncthreads();
+}
+
+template <int F, int W, int NC, bool GMEM_X, bool PEAK, bool SEG>
+__global__ void __launch_bounds__(kWarp * W, 1) spiir_scan_fused_kernel(const ScanFusedParams sp)
+{
+    const int seg = blockIdx.y, item = blockIdx.x;
+    const bool has_pass1 = seg + 1 < sp.n_seg;                    // the last segment's zero-state end values are never used
+    {
+        // The window [t0 - w0, t0 + nseg) of this segment: history from the bank's tape, the call's own samples straight from
+        // the caller's buffer (the kernel appends them to the tape itself, so a call is this one launch and nothing else).
+        const FilterParams& p = sp.pass2;
+        const int64_t t0 = (int64_t)seg * p.seg_len;
+        const int nseg = (int)min(p.seg_len, p.n - t0);
+        const int win_len = p.w0 + nseg;
+        int64_t cstride;
+        filter_smem_bytes(W, NC, win_len, GMEM_X, &cstride);
+        extern __shared__ __align__(16) float smem[];
+        const int64_t first = t0 - p.w0;                         // call-relative sample index of window element 0
+        for (int k = threadIdx.x; k < (int)cstride; k += kWarp * W) {
+            const int64_t i = first + k;
+            smem[k] = k < win_len ? (i < 0 ? p.xwin[t0 + k] : sp.xnew[i]) : 0.f;
+        }
+        if (item == 0)
+            for (int k = threadIdx.x; k < nseg; k += kWarp * W) sp.append[t0 + k] = sp.xnew[t0 + k];
+        __syncthreads();
+        make_shifted_copies<NC>(smem, cstride, threadIdx.x, kWarp * W);
+        __syncthreads();
+    }
+    if (has_pass1) filter_body<F, W, NC, GMEM_X, 1, PEAK, SEG>(sp.pass1, seg, item, sp.pass1.n_items, true);
+    grid_barrier(sp.barrier, sp.target);
+    {
+        // true start states of every segment, one slot per thread over the whole grid (the chain over the segments of a
+        // slot is sequential, the slots are independent): c_0 = carried state, c_{q+1} = a1^L c_q + z_q in double
+        const FilterParams& p = sp.pass1;
+        const int64_t L = p.seg_len;
+        const int64_t n_threads = (int64_t)gridDim.x * gridDim.y * blockDim.x;
+        const int64_t per_tile = (int64_t)F * kWarp;
+        for (int64_t s = ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x; s < sp.n_slots; s += n_threads) {
+            const float* rec = p.coef + (s / per_tile) * 5 * per_tile + s % per_tile;
+            // the chain over the segments is dependent, the loads of the end states are not: two batches of kB in flight,
+            // the first one requested before the power is worked out
+            constexpr int kB = 8;
+            float2 za[kB], zb[kB];
+            const float* zs = sp.z + 2 * s;
+            const int64_t zstride = 2 * sp.n_slots;
+            const int n_z = sp.n_seg - 1;
+            auto fetch = [&](float2 (&zz)[kB], int q0) {
+#pragma unroll
+                for (int i = 0; i < kB; ++i)
+                    zz[i] = __ldcg(reinterpret_cast<const float2*>(zs + (int64_t)min(q0 + i, n_z - 1) * zstride));
+            };
+            if (n_z > 0) fetch(za, 0);
+            float cr = sp.y[2 * s], ci = sp.y[2 * s + 1];
+            double pr = 1.0, pi = 0.0, br = (double)rec[0], bi = (double)rec[per_tile];
+            for (int64_t e = L; e > 0; e >>= 1) {                              // a1^L by binary powering in double
+                if (e & 1) { const double tr = pr * br - pi * bi, ti = pr * bi + pi * br; pr = tr; pi = ti; }
+                const double tr = br * br - bi * bi, ti = 2.0 * br * bi; br = tr; bi = ti;
+            }
+            const float Ar = (float)pr, Ai = (float)pi;                        // a1^L: from double, rounded once
+            *reinterpret_cast<float2*>(sp.cbuf + 2 * s) = make_float2(cr, ci);
+            auto chain = [&](const float2 (&zz)[kB], int q0) {
+#pragma unroll
+                for (int i = 0; i < kB; ++i) {
+                    if (q0 + i < n_z) {
+                        scan_carry_step(Ar, Ai, zz[i].x, zz[i].y, cr, ci);
+                        *reinterpret_cast<float2*>(sp.cbuf + (int64_t)(q0 + i + 1) * zstride + 2 * s) = make_float2(cr, ci);
+                    }
+                }
+            };
+            for (int q0 = 0; q0 < n_z; q0 += 2 * kB) {
+                if (q0 + kB < n_z) fetch(zb, q0 + kB);
+                chain(za, q0);
+                if (q0 + 2 * kB < n_z) fetch(za, q0 + 2 * kB);
+                if (q0 + kB < n_z) chain(zb, q0 + kB);
+            }
+        }
+    }
+    grid_barrier(sp.barrier, sp.target + (unsigned long long)gridDim.x * gridDim.y);
+    filter_body<F, W, NC, GMEM_X, 1, PEAK, SEG>(sp.pass2, seg, item, sp.pass2.n_items, true);
 }
 
 // ---- tiny-chunk streaming (SPIIR_PATH_STREAM, n <= kStreamMax samples per call).
@@ -652,15 +783,15 @@ __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, con
 
 // ---- time-parallel scan: carry combine.  For every slot, given the carried state c_0 = y and the
 // zero-state end values z_p of segments p = 0..P-2 (all of length seg_len), produce the true start
-// states c_{p+1} = a1^seg_len * c_p + z_p.  Powers and the combine are evaluated in double from the
-// float32 a1 (SURVEY.md section 8(c) finding F2), then rounded once to float32.
+// states c_{p+1} = a1^seg_len * c_p + z_p.  The power is evaluated in double from the float32 a1 by binary powering and
+// rounded once to float32 (SURVEY.md section 8(c) finding F2: 2.7e-6 of max|SNR| with multipliers from double against
+// 3.3e-5 with FP32 repeated squaring); the combine itself is the same FP32 complex multiply-add a filter step is.
 __global__ void spiir_scan_carry_kernel(const float* __restrict__ coef, int32_t F,
                                         const float* __restrict__ y, const float* __restrict__ z,
                                         float* __restrict__ c, int64_t n_slots, int32_t n_seg, int64_t seg_len)
 {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_slots) return;
-    // a^L by binary exponentiation in double
     const int64_t per_tile = (int64_t)F * kWarp;
     const float* rec = coef + (s / per_tile) * 5 * per_tile + s % per_tile;
     double pr = 1.0, pi = 0.0, br = (double)rec[0], bi = (double)rec[per_tile];
@@ -668,30 +799,26 @@ __global__ void spiir_scan_carry_kernel(const float* __restrict__ coef, int32_t 
         if (e & 1) { const double tr = pr * br - pi * bi, ti = pr * bi + pi * br; pr = tr; pi = ti; }
         const double tr = br * br - bi * bi, ti = 2.0 * br * bi; br = tr; bi = ti;
     }
-    double cr = (double)y[2 * s], ci = (double)y[2 * s + 1];
+    const float Ar = (float)pr, Ai = (float)pi;
+    float cr = y[2 * s], ci = y[2 * s + 1];
     // c[0] is the carried state itself (segment 0 starts from it)
-    c[2 * s] = (float)cr;
-    c[2 * s + 1] = (float)ci;
+    c[2 * s] = cr;
+    c[2 * s + 1] = ci;
     // the carries are a dependent chain, the loads of z are not: fetch them kB at a time ahead of the chain
-    constexpr int kB = 16;
+    constexpr int kB = 8;
     for (int32_t q0 = 0; q0 + 1 < n_seg; q0 += kB) {
-        float zr[kB], zi[kB];
+        float2 zz[kB];
 #pragma unroll
         for (int i = 0; i < kB; ++i) {
             const int32_t q = min(q0 + i, n_seg - 2);
-            zr[i] = z[(int64_t)q * 2 * n_slots + 2 * s];
-            zi[i] = z[(int64_t)q * 2 * n_slots + 2 * s + 1];
+            zz[i] = *reinterpret_cast<const float2*>(z + (int64_t)q * 2 * n_slots + 2 * s);
         }
 #pragma unroll
         for (int i = 0; i < kB; ++i) {
             const int32_t q = q0 + i;
             if (q + 1 < n_seg) {
-                const double nr = pr * cr - pi * ci + (double)zr[i], ni = pr * ci + pi * cr + (double)zi[i];
-                // continue from the float32-rounded carry: that is the state segment q+1 really starts from
-                cr = (double)(float)nr;
-                ci = (double)(float)ni;
-                c[(int64_t)(q + 1) * 2 * n_slots + 2 * s] = (float)nr;
-                c[(int64_t)(q + 1) * 2 * n_slots + 2 * s + 1] = (float)ni;
+                scan_carry_step(Ar, Ai, zz[i].x, zz[i].y, cr, ci);
+                *reinterpret_cast<float2*>(c + (int64_t)(q + 1) * 2 * n_slots + 2 * s) = make_float2(cr, ci);
             }
         }
     }

@@ -87,12 +87,12 @@ def test_every_invalid_blocking_pair_is_rejected_at_create(pkg):
         with pytest.raises(pkg.SpiirError) as ei:
             pkg.spiir_bank_create(off, a1, b0, d, options=pkg.SpiirOptions(path=pkg.PATH_STREAM, filters_per_thread=F))
         assert ei.value.code == -1
-    # reserved must be 0
+    # scan_launches is 0 or 3
     opt = pkg.SpiirOptions()
-    opt.reserved[0] = 7
+    opt.scan_launches = 7
     with pytest.raises(pkg.SpiirError) as ei:
         pkg.spiir_bank_create(off, a1, b0, d, options=opt)
-    assert ei.value.code == -1 and "reserved" in str(ei.value)
+    assert ei.value.code == -1 and "scan_launches" in str(ei.value)
 
 
 def test_fails_loudly_without_a_gpu(pkg):

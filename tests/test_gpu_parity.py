@@ -32,14 +32,16 @@ def env():
     return pkg, oracle, torch
 
 
-def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=False, small=0, device_result=False):
+def run_gpu(env, inp, chunks=None, path=0, F=0, segments=0, rows=None, host=False, small=0, device_result=False,
+            scan_launches=0):
     """Filter inp.x through a fresh bank in the given chunking; returns complex64 [T or len(rows), N]
     (numpy, or the CUDA tensor itself with device_result)."""
     pkg, _, torch = env
     N = inp.n_samples
     chunks = [N] if chunks is None else list(chunks)
     assert sum(chunks) == N
-    opt = pkg.SpiirOptions(path=path, filters_per_thread=F, scan_segments=segments, small_templates=small)
+    opt = pkg.SpiirOptions(path=path, filters_per_thread=F, scan_segments=segments, small_templates=small,
+                           scan_launches=scan_launches)
     with pkg.SpiirBank(inp.offsets, inp.a1, inp.b0, inp.delays, 0, opt) as bank:
         if host:
             out = np.empty((inp.n_templates, N), dtype=np.complex64)
@@ -105,6 +107,24 @@ def test_p7_golden_vector_bitwise(env, path, F):
     assert np.array_equal(got[0], np.array(rows, dtype=np.complex64))
     got = run_gpu(env, inp, chunks=[3, 1, 4], path=path, F=F)
     assert np.array_equal(got[0], np.array(rows, dtype=np.complex64))
+
+
+# ------------------------------------------------------------------ time-parallel path: one launch == three launches
+@pytest.mark.parametrize("cfg,chunks,F", [(0, None, 0), (0, [1000, 24, 3000, 72], 0), (1, [4096] * 16, 0), (1, None, 0),
+                                          (1, [30000, 35536], 16), (0, [2048, 2048], 1)])
+def test_scan_single_launch_equals_three_launches(env, cfg, chunks, F):
+    """The cooperative single-launch form of the time-parallel path (carry pass, grid barrier, carries in double, output
+    pass) does the arithmetic of the three-launch form in the same order: bitwise equal, one kernel per call."""
+    pkg = env[0]
+    inp = spiir_inputs.make_config(cfg)
+    n0 = pkg.spiir_kernel_launches()
+    one = run_gpu(env, inp, chunks=chunks, path=2, F=F, device_result=True)
+    n1 = pkg.spiir_kernel_launches()
+    three = run_gpu(env, inp, chunks=chunks, path=2, F=F, scan_launches=3, device_result=True)
+    n2 = pkg.spiir_kernel_launches()
+    assert env[2].equal(one.view(env[2].float32), three.view(env[2].float32))
+    if F == 0:
+        assert n1 - n0 < n2 - n1, "the single-launch form was not taken"
 
 
 # ------------------------------------------------------------------ configs 0 and 1, full bank, every element
