@@ -45,8 +45,8 @@ FLOPS_PER_FILTER_SAMPLE = 12          # complex*complex 6 + real*complex 2 + com
 N_SM, LANES, BOOST_HZ = 148, 128, 1.965e9   # B200: SMs x FP32 lanes x 2 flops x clocks.max.sm (MEASURED_PEAKS.json sm_max_mhz)
 FP32_PEAK_TFLOPS = N_SM * LANES * 2 * BOOST_HZ / 1e12    # 74.4 TFLOP/s, derivation in DESIGN.md section 7
 # dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch (cfg3, default blocking, 8192 samples)
-# from the committed ncu --set full capture profiles/r01c_filter_kernel_full.md: 119.1 MB + 244.9 MB
-NCU_TRAFFIC_CFG3_LAUNCH = 364.0e6
+# from the committed ncu --set full capture profiles/r02_filter_kernel_full.md: 119.3 MB + 244.6 MB
+NCU_TRAFFIC_CFG3_LAUNCH = 363.8e6
 # the same for one spiir_stream_kernel launch of cfg4 (16 samples), profiles/r01c_cfg4_stream_launches.md: 144.7 MB + 18.8 MB
 NCU_TRAFFIC_CFG4_LAUNCH = 163.5e6
 
