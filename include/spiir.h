@@ -81,9 +81,13 @@ typedef struct spiir_options {
     int32_t small_templates;    /* templates of <= 128 filters sharing warp tiles (sub-warp segments):
                                    0 = choose, 1 = on (forces the (8,16) blocking), 2 = off.  Not used with
                                    SPIIR_PATH_STREAM. */
-    int32_t scan_launches;      /* SPIIR_PATH_SCAN: 0 = choose (one cooperative launch per call when every CTA of the
-                                   items x segments grid is resident, else three), 3 = always the three-launch form
-                                   (carry pass, carry scan, output pass); any other value is SPIIR_EINVAL */
+    int32_t scan_launches;      /* kernel launches per call of the two low-latency paths.  0 = choose: SPIIR_PATH_SCAN takes
+                                   one cooperative launch when every CTA of the items x segments grid is resident (else
+                                   three), SPIIR_PATH_STREAM a tile kernel + a combine kernel chained by programmatic
+                                   dependent launch (measured faster than one launch).  1 = one launch wherever the
+                                   grid can meet at a barrier (both paths).  3 = always separate kernels (scan: carry
+                                   pass, carry scan, output pass).  All forms of a path give the same bits.  Any other
+                                   value is SPIIR_EINVAL */
 } spiir_options;
 
 /* Build a bank.  All pointers are HOST pointers; the arrays are copied, the caller keeps ownership.

@@ -28,6 +28,9 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#ifdef SPIIR_SCAN_TIMING
+#include <cstdio>
+#endif
 
 #include "spiir_layout.hpp"
 
@@ -175,6 +178,22 @@ __device__ __forceinline__ void mbar_wait(u64* bar, unsigned parity)
         "WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
         " @p bra DONE_%=;\n bra WAIT_%=;\n"
         "DONE_%=:\n}" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+
+// Grid-wide barrier of a kernel whose CTAs are all resident: a monotonic arrival counter in global memory, `target` = its value
+// once every CTA of this launch has arrived (the host keeps the running total, so the counter is never reset).
+__device__ __forceinline__ void grid_barrier(unsigned long long* counter, unsigned long long target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();                                                      // this CTA's end states are visible device-wide
+        atomicAdd(counter, 1ull);
+        unsigned long long v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(counter) : "memory");
+        } while (v < target);
+    }
+    __syncthreads();
 }
 
 // Window staging (north_star subsystem (3): "stages the delayed input window into shared
@@ -544,23 +563,21 @@ struct ScanFusedParams {
     unsigned long long target;       // its value when every CTA of this launch has arrived at the first barrier
 };
 
-__device__ __forceinline__ void grid_barrier(unsigned long long* counter, unsigned long long target)
-{
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();                                                      // this CTA's end states are visible device-wide
-        atomicAdd(counter, 1ull);
-        unsigned long long v;
-        do {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(counter) : "memory");
-        } while (v < target);
-    }
-    __syncthreads();
-}
+// -DSPIIR_SCAN_TIMING: the first and the last segment's CTA of item 0 print the duration of every phase (%globaltimer, ns)
+// for the first launches of a bank -- the launch-gap / phase instrument of profiles/r02_scan_phases.md (no nsys in the image).
+#ifdef SPIIR_SCAN_TIMING
+#define SPIIR_STAMP(k) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(stamp[k]))
+#else
+#define SPIIR_STAMP(k)
+#endif
 
 template <int F, int W, int NC, bool GMEM_X, bool PEAK, bool SEG>
 __global__ void __launch_bounds__(kWarp * W, 1) spiir_scan_fused_kernel(const ScanFusedParams sp)
 {
+#ifdef SPIIR_SCAN_TIMING
+    unsigned long long stamp[6];
+#endif
+    SPIIR_STAMP(0);
     const int seg = blockIdx.y, item = blockIdx.x;
     const bool has_pass1 = seg + 1 < sp.n_seg;                    // the last segment's zero-state end values are never used
     {
@@ -584,8 +601,11 @@ __global__ void __launch_bounds__(kWarp * W, 1) spiir_scan_fused_kernel(const Sc
         make_shifted_copies<NC>(smem, cstride, threadIdx.x, kWarp * W);
         __syncthreads();
     }
+    SPIIR_STAMP(1);
     if (has_pass1) filter_body<F, W, NC, GMEM_X, 1, PEAK, SEG>(sp.pass1, seg, item, sp.pass1.n_items, true);
+    SPIIR_STAMP(2);
     grid_barrier(sp.barrier, sp.target);
+    SPIIR_STAMP(3);
     {
         // true start states of every segment, one slot per thread over the whole grid (the chain over the segments of a
         // slot is sequential, the slots are independent): c_0 = carried state, c_{q+1} = a1^L c_q + z_q in double
@@ -634,7 +654,14 @@ __global__ void __launch_bounds__(kWarp * W, 1) spiir_scan_fused_kernel(const Sc
         }
     }
     grid_barrier(sp.barrier, sp.target + (unsigned long long)gridDim.x * gridDim.y);
+    SPIIR_STAMP(4);
     filter_body<F, W, NC, GMEM_X, 1, PEAK, SEG>(sp.pass2, seg, item, sp.pass2.n_items, true);
+    SPIIR_STAMP(5);
+#ifdef SPIIR_SCAN_TIMING
+    if (threadIdx.x == 0 && item == 0 && (seg == 0 || seg == sp.n_seg - 1) && sp.target < 40ull * gridDim.x * gridDim.y)
+        printf("scan launch, segment %d of %d: window %llu  carry pass %llu  barrier %llu  carries + barrier %llu  output pass %llu ns\n",
+               seg, sp.n_seg, stamp[1] - stamp[0], stamp[2] - stamp[1], stamp[3] - stamp[2], stamp[4] - stamp[3], stamp[5] - stamp[4]);
+#endif
 }
 
 // ---- tiny-chunk streaming (SPIIR_PATH_STREAM, n <= kStreamMax samples per call).
@@ -656,7 +683,38 @@ struct StreamParams {
     float* append;                // where CTA 0 stores the chunk for later calls (the bank's tape); nullptr: already there
     int64_t n_tiles;
     u64* scratch;                 // [n_tiles][kStreamMax] partial sums of every warp tile
+    // combine phase of the same launch (barrier == nullptr: a separate spiir_stream_combine_kernel follows instead)
+    const int64_t* tile_begin;    // [n_templates + 1] first warp tile of every template
+    int32_t n_templates;
+    float* snr; int64_t ld;       // complex64 rows
+    u64* peaks;                   // fused trigger reduction or nullptr
+    unsigned long long* barrier;  // grid-wide barrier between the two phases
+    unsigned long long target;
 };
+
+// SNR[t][j] = sum over the warp tiles of template t, in tile order, of scratch[tile][j] (fixed order -> bitwise reproducible,
+// independent of a template's position in the bank).
+__device__ __forceinline__ void stream_combine_one(const u64* __restrict__ scratch, const int64_t* __restrict__ tile_begin, int64_t i,
+                                                   int32_t n, float* __restrict__ snr, int64_t ld, u64* __restrict__ peaks, bool cg)
+{
+    const int32_t t = (int32_t)(i / n), j = (int32_t)(i % n);
+    const int64_t t0 = tile_begin[t], t1 = tile_begin[t + 1];
+    u64 acc = cg ? __ldcg(scratch + t0 * kStreamMax + j) : scratch[t0 * kStreamMax + j];
+    // loads 16 tiles ahead of the (ordered) additions: the chain of adds is short, the chain of L2 latencies is not
+    for (int64_t tile = t0 + 1; tile < t1; tile += 16) {
+        u64 v[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const u64* src = scratch + (tile + q) * kStreamMax + j;
+            v[q] = (tile + q < t1) ? (cg ? __ldcg(src) : *src) : 0ull;
+        }
+#pragma unroll
+        for (int q = 0; q < 16; ++q)
+            if (tile + q < t1) acc = fadd2(acc, v[q]);
+    }
+    if (snr) reinterpret_cast<u64*>(snr)[(int64_t)t * ld + j] = acc;
+    if (peaks) atomicMax(peaks + t, peak_key(acc, j));
+}
 
 __host__ __device__ inline size_t stream_smem_bytes(int F, int NC, int64_t win_len, int64_t* cstride_out)
 {
@@ -754,31 +812,27 @@ __global__ void __launch_bounds__(kWarp * stream_warps(F), 1) spiir_stream_kerne
 #pragma unroll
         for (int f = 0; f < F; ++f) *reinterpret_cast<u64*>(p.y + 2 * (s0 + f * kWarp)) = Y[f];
     }
+    if (p.barrier) {
+        // second phase of the same launch: every CTA is resident (grid <= SMs x occupancy), so the grid can meet at a
+        // barrier; the partial rows are then summed per (template, sample) by all threads of the grid
+        asm volatile("griddepcontrol.launch_dependents;");     // the next call's kernel may be set up (it waits itself)
+        grid_barrier(p.barrier, p.target);
+        const int64_t total = (int64_t)p.n_templates * p.n;
+        for (int64_t i = (int64_t)blockIdx.x * kThreads + tid; i < total; i += (int64_t)gridDim.x * kThreads)
+            stream_combine_one(p.scratch, p.tile_begin, i, p.n, p.snr, p.ld, p.peaks, true);
+    }
 }
 
-// SNR[t][j] = sum over the warp tiles of template t, in tile order, of scratch[tile][j].  One thread per (t, j).
+// The combine as a kernel of its own (one thread per (t, j)): used when the streaming kernel's grid cannot meet at a barrier.
 __global__ void spiir_stream_combine_kernel(const u64* __restrict__ scratch, const int64_t* __restrict__ tile_begin,
                                             int32_t n_templates, int32_t n, float* __restrict__ snr, int64_t ld,
                                             u64* __restrict__ peaks)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= (int64_t)n_templates * n) return;
-    const int32_t t = (int32_t)(i / n), j = (int32_t)(i % n);
-    const int64_t t0 = tile_begin[t], t1 = tile_begin[t + 1];
     asm volatile("griddepcontrol.wait;" ::: "memory");     // launched early (PDL): the streaming kernel's rows from here on
     asm volatile("griddepcontrol.launch_dependents;");     // the next call's streaming kernel may be set up (it waits itself)
-    u64 acc = scratch[t0 * kStreamMax + j];
-    // loads 16 tiles ahead of the (ordered) additions: the chain of adds is short, the chain of L2 latencies is not
-    for (int64_t tile = t0 + 1; tile < t1; tile += 16) {
-        u64 v[16];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) v[q] = (tile + q < t1) ? scratch[(tile + q) * kStreamMax + j] : 0ull;
-#pragma unroll
-        for (int q = 0; q < 16; ++q)
-            if (tile + q < t1) acc = fadd2(acc, v[q]);
-    }
-    if (snr) reinterpret_cast<u64*>(snr)[(int64_t)t * ld + j] = acc;
-    if (peaks) atomicMax(peaks + t, peak_key(acc, j));
+    stream_combine_one(scratch, tile_begin, i, n, snr, ld, peaks, false);
 }
 
 // ---- time-parallel scan: carry combine.  For every slot, given the carried state c_0 = y and the

@@ -87,7 +87,7 @@ def test_every_invalid_blocking_pair_is_rejected_at_create(pkg):
         with pytest.raises(pkg.SpiirError) as ei:
             pkg.spiir_bank_create(off, a1, b0, d, options=pkg.SpiirOptions(path=pkg.PATH_STREAM, filters_per_thread=F))
         assert ei.value.code == -1
-    # scan_launches is 0 or 3
+    # scan_launches is 0, 1 or 3
     opt = pkg.SpiirOptions()
     opt.scan_launches = 7
     with pytest.raises(pkg.SpiirError) as ei:

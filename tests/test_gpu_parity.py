@@ -127,6 +127,21 @@ def test_scan_single_launch_equals_three_launches(env, cfg, chunks, F):
         assert n1 - n0 < n2 - n1, "the single-launch form was not taken"
 
 
+def test_stream_single_launch_equals_two_launches(env):
+    """Tiny-chunk path: tile phase + grid barrier + combine phase in one launch == tile kernel + combine kernel."""
+    pkg = env[0]
+    inp = spiir_inputs.make_random_bank(77, [700, 64, 2048, 130, 1, 300, 1500, 90], 16 * 40 + 13, d_max=900)
+    chunks = [16] * 40 + [13]
+    n0 = pkg.spiir_kernel_launches()
+    one = run_gpu(env, inp, chunks=chunks, path=3, scan_launches=1, device_result=True)
+    n1 = pkg.spiir_kernel_launches()
+    two = run_gpu(env, inp, chunks=chunks, path=3, device_result=True)
+    n2 = pkg.spiir_kernel_launches()
+    assert env[2].equal(one.view(env[2].float32), two.view(env[2].float32))
+    assert n1 - n0 == len(chunks) and n2 - n1 == 2 * len(chunks)
+    check(one.cpu().numpy(), env[1].run_inputs(inp))
+
+
 # ------------------------------------------------------------------ configs 0 and 1, full bank, every element
 @pytest.mark.parametrize("path", [0, 1, 2])
 def test_cfg0_full(env, path):
