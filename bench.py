@@ -47,8 +47,8 @@ FP32_PEAK_TFLOPS = N_SM * LANES * 2 * BOOST_HZ / 1e12    # 74.4 TFLOP/s, derivat
 # dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch (cfg3, default blocking, 8192 samples)
 # from the committed ncu --set full capture profiles/r02_filter_kernel_full.md: 119.3 MB + 244.6 MB
 NCU_TRAFFIC_CFG3_LAUNCH = 363.8e6
-# the same for one spiir_stream_kernel launch of cfg4 (16 samples), profiles/r01c_cfg4_stream_launches.md: 144.7 MB + 18.8 MB
-NCU_TRAFFIC_CFG4_LAUNCH = 163.5e6
+# the same for one spiir_stream_kernel launch of cfg4 (16 samples), profiles/r02_cfg4_stream_launches.md: 144.6 MB + 18.2 MB
+NCU_TRAFFIC_CFG4_LAUNCH = 162.8e6
 
 
 def measured_hbm_peak():
