@@ -786,6 +786,8 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
                 continue;
             }
 
+            // F = 16 keeps 2 copies: its LDS.128 variant needs all 255 registers and measures 8 % slower (cfg2: 43.2 -> 46.6 %)
+            if (nc == 4 && bk->F == 16) continue;
             if ((hist + kMinSub) * 4 * nc <= room) { bk->NC = nc; break; }
         }
         if (o.window_copies == 1 || o.window_copies == 2 || o.window_copies == 4)
