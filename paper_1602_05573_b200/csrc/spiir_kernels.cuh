@@ -85,7 +85,8 @@ struct FilterParams {
 // The delayed input comes from NC shifted copies of the window (copy c holds win[i + c]), so that every
 // filter reads NC consecutive samples with one aligned LDS.32 / LDS.64 / LDS.128 (xo[f] already points
 // into the copy that makes its loads aligned).
-template <int F, int NC, bool FULL>
+// SUMS = false: states only (carry pass of the single-launch time-parallel kernel), S is left untouched.
+template <int F, int NC, bool FULL, bool SUMS = true>
 __device__ __forceinline__ void tile_step(const float* __restrict__ xs, const int (&xo)[F], const float (&ar)[F],
                                           const u64 (&AI)[F], const u64 (&B)[F], u64 (&Y)[F], u64 (&S)[kTT],
                                           int tb, int nv)
@@ -119,11 +120,13 @@ __device__ __forceinline__ void tile_step(const float* __restrict__ xs, const in
                     t = ffma2(AI[f], pack2(yi, yr), t);
                     Y[f] = ffma2(pack2(ar[f], ar[f]), Y[f], t);
                     // S_j = ((Y_0 + Y_1) + Y_2) + ...: the first two outputs are added directly, no copy of Y_0
-                    if (F == 1) S[j] = Y[0];
-                    else if (f == 1) S[j] = fadd2(Y[0], Y[1]);
-                    else if (f > 1) S[j] = fadd2(S[j], Y[f]);
+                    if (SUMS) {
+                        if (F == 1) S[j] = Y[0];
+                        else if (f == 1) S[j] = fadd2(Y[0], Y[1]);
+                        else if (f > 1) S[j] = fadd2(S[j], Y[f]);
+                    }
                 }
-            } else {
+            } else if (SUMS) {
                 S[j] = 0ull;
             }
         }
@@ -373,7 +376,8 @@ __host__ __device__ inline size_t filter_smem_bytes(int W, int NC, int64_t win_l
 // SEG compiles the shared-tile path for banks of small templates in.
 // The body of the blocked kernel for time segment `seg`, items item0, item0 + item_stride, ...; `staged` = the window of this
 // segment is already in shared memory (second pass of the fused time-parallel kernel).
-template <int F, int W, int NC, bool GMEM_X, int MINB, bool PEAK, bool SEG>
+// SUMS = false compiles the sums, the reduction and the output out (carry pass).
+template <int F, int W, int NC, bool GMEM_X, int MINB, bool PEAK, bool SEG, bool SUMS = true>
 __device__ __forceinline__ void filter_body(const FilterParams& p, const int seg, const int item0, const int item_stride,
                                             const bool staged)
 {
@@ -401,7 +405,7 @@ __device__ __forceinline__ void filter_body(const FilterParams& p, const int seg
     const int staged_floats = (win_len + 3) / 4 * 4;                           // floats the bulk copy brings (16-byte units)
     if (!GMEM_X && !staged && tid == 0) stage_window_issue(smem, p.xwin + t0, (unsigned)staged_floats * 4u, stage_bar);   // t0, xwin: 16-byte aligned
     // per-template hand-over without any CTA-wide barrier: only where one CTA owns the SM and all rounds have one shape
-    const bool sums = PEAK ? (p.snr || p.peaks) : (p.snr != nullptr);                                        // false: carry pass, states only
+    const bool sums = SUMS && (PEAK ? (p.snr || p.peaks) : (p.snr != nullptr));                              // false: carry pass, states only
     const bool async = kAsync && p.uniform_groups && sums;
     if (async && tid < W) {
         const int first = p.canon[2 * tid], count = p.canon[2 * tid + 1];
@@ -494,8 +498,8 @@ __device__ __forceinline__ void filter_body(const FilterParams& p, const int seg
                         for (int tt = 0; tt < ns; tt += kTT) {
                             u64 S[kTT];
                             const int nv = ns - tt;
-                            if (nv >= kTT) tile_step<F, NC, true>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
-                            else tile_step<F, NC, false>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
+                            if (nv >= kTT) tile_step<F, NC, true, SUMS>(xs, xo, ar, AI, B, Y, S, (int)st + tt, kTT);
+                            else tile_step<F, NC, false, SUMS>(xs, xo, ar, AI, B, Y, S, (int)st + tt, nv);
                             if (sums) {
                                 if (SEG && seg_w) {
                                     seg_reduce_store<PEAK>(S, mytr, lane, seg_w, seg_n, nv, (!PEAK || out_row) ? out_row + st + tt : nullptr, p.ld,
@@ -602,7 +606,7 @@ __global__ void __launch_bounds__(kWarp * W, 1) spiir_scan_fused_kernel(const Sc
         __syncthreads();
     }
     SPIIR_STAMP(1);
-    if (has_pass1) filter_body<F, W, NC, GMEM_X, 1, PEAK, SEG>(sp.pass1, seg, item, sp.pass1.n_items, true);
+    if (has_pass1) filter_body<F, W, NC, GMEM_X, 1, PEAK, SEG, false>(sp.pass1, seg, item, sp.pass1.n_items, true);
     SPIIR_STAMP(2);
     grid_barrier(sp.barrier, sp.target);
     SPIIR_STAMP(3);
