@@ -281,7 +281,8 @@ const void* select_scan_fused_kernel(int F, int W, int NC)
     return nullptr;
 }
 
-int default_warps(int F) { return F >= 16 ? 8 : (F == 8 ? 16 : 32); }
+// F = 4 takes 16 warps: with 32 (64 registers per thread) the body spills and measures 34 % of peak against 41 %
+int default_warps(int F) { return F >= 16 ? 8 : (F >= 4 ? 16 : 32); }
 
 // shared memory besides the window copies
 // variants compiled for several CTAs per SM keep the CTA-wide barrier and need only 2 partial-sum buffers
