@@ -504,7 +504,9 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     // ---------------------------------------------------- time-parallel scan path (north_star (4))
     NvtxRange range("spiir_filter: time-parallel path");
     bk->last_path = SPIIR_PATH_SCAN;
-    int64_t seg_len = round_up((n + n_seg - 1) / n_seg, kTS);
+    // segments of >= 64 samples in steps of 16 (two register tiles; keeps every segment's window 16-byte aligned): cfg1's
+    // 4096-sample call over 4 items becomes 37 segments of 112 samples = 148 CTAs instead of 32 of 128 = 128 CTAs
+    int64_t seg_len = std::max<int64_t>(kTS, round_up((n + n_seg - 1) / n_seg, 16));
     if (!gmem && w0 + seg_len > max_win) seg_len = std::max<int64_t>(kTS, (max_win - w0) / kTS * kTS);
     n_seg = (n + seg_len - 1) / seg_len;
     if (n_seg > bk->scan_cap_seg) {
