@@ -85,7 +85,9 @@ typedef struct spiir_options {
                                    one cooperative launch when every CTA of the items x segments grid is resident (else
                                    three), SPIIR_PATH_STREAM a tile kernel + a combine kernel chained by programmatic
                                    dependent launch (measured faster than one launch).  1 = one launch wherever the
-                                   grid can meet at a barrier (both paths).  3 = always separate kernels (scan: carry
+                                   grid can meet at a barrier (both paths; the streaming kernel is then a plain launch of
+                                   at most SMs x occupancy CTAs that spin at a grid-wide barrier: do not run it beside
+                                   other kernels that keep SMs occupied indefinitely).  3 = always separate kernels (scan: carry
                                    pass, carry scan, output pass).  All forms of a path give the same bits.  Any other
                                    value is SPIIR_EINVAL */
 } spiir_options;
