@@ -101,7 +101,7 @@ def decode(ins: Ins) -> bool:
             if r != RZ:
                 ins.reads += list(range(r, r + w))
         return True
-    m = re.match(r"(LDS(?:\.\d+)?)\s+R(\d+), \[R(\d+)(?:\+0x[0-9a-f]+)?\]$", ins.text)
+    m = re.match(r"(LDS(?:\.\d+)?)\s+R(\d+), \[R(\d+)(?:\+-?0x[0-9a-f]+)?\]$", ins.text)
     if m:
         width = {"LDS": 1, "LDS.64": 2, "LDS.128": 4}.get(m.group(1))
         if width is None:
@@ -396,7 +396,7 @@ def interpret(block, R):
                         res = tuple(np.float32(np.float64(A[i]) * np.float64(B[i]) + np.float64(C[i])) for i in range(2))
                 R[d], R[d + 1] = u32(res[0]), u32(res[1])
             elif x.op == "LDS":
-                m = re.match(r"LDS(?:\.(\d+))?\s+R(\d+), \[R(\d+)(?:\+0x([0-9a-f]+))?\]", x.text)
+                m = re.match(r"LDS(?:\.(\d+))?\s+R(\d+), \[R(\d+)(?:\+(-?0x[0-9a-f]+))?\]", x.text)
                 w = {None: 1, "64": 2, "128": 4}[m.group(1)]
                 addr = (int(R[int(m.group(3))]) + int(m.group(4) or "0", 16)) & 0xffffffff
                 for k in range(w):
