@@ -132,6 +132,23 @@ int spiir_filter(spiir_bank *bank, const float *x_dev, int64_t n, float *snr_dev
 int spiir_filter_peaks(spiir_bank *bank, const float *x_dev, int64_t n, float *snr_dev, int64_t ld,
                        float *power_dev, int32_t *index_dev, void *stream);
 
+/* spiir_filter for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): one tiny-chunk call of a bank created with SPIIR_PATH_STREAM, same arguments, same results (the same two
+ * kernels; bitwise equal to spiir_filter), but the per-tile partial sums go to a file-scope device array of the library
+ * instead of a buffer from cudaMalloc.  The call reaches no cudaMalloc, cudaFree or allocating library routine.
+ *   limits   n <= 64 samples; the bank has at most 8192 warp tiles (32 x filters_per_thread filter slots each: 1 048 576
+ *            slots at the streaming default of 4 filters per thread); the array is 4 MiB and every GPU that loads the
+ *            library holds it until exit.  Anything beyond returns SPIIR_EINVAL with a message saying which limit;
+ *            so does a call that would have to create an event (a bank moved to another stream for the first time).
+ *   set-up   the first call on a device looks the array's address up (cudaGetSymbolAddress) and sets the kernel's
+ *            attributes: make it before a graph capture starts.
+ *   sharing  all banks and calls on a device share the array, which keeps the last call's contents.  Nothing has to start
+ *            at zero (every row the combine pass reads is written by the tile pass of the same call), but calls that
+ *            overlap on the GPU -- two banks on different streams -- race on it: serialise them.
+ * May be mixed with spiir_filter on the same bank (state and history carry over either way). */
+int spiir_filter_static(spiir_bank *bank, const float *x_dev, int64_t n, float *snr_dev, int64_t ld,
+                        void *stream);
+
 /* Same operation with HOST buffers (the end-to-end entry): copies x to the device, filters, copies
  * SNR[t][0..n) back into snr_host (row stride ld), overlapping copies and kernels internally.
  * Buffers may be pageable or pinned.  Returns after the results are in snr_host. */

@@ -5,7 +5,7 @@ here have the same names as the C entry points and only marshal arguments; every
 runs in the library's CUDA kernels.  There is no CPU fallback: without the built library or without a
 CUDA device the calls raise.
 """
-from .binding import (SpiirError, SpiirOptions, SpiirBank, spiir_bank_create, spiir_filter, spiir_filter_prepared,  # noqa: F401
+from .binding import (SpiirError, SpiirOptions, SpiirBank, spiir_bank_create, spiir_filter, spiir_filter_prepared, spiir_filter_static,  # noqa: F401
                       spiir_filter_peaks, spiir_filter_host, spiir_filter_host_async, spiir_bank_host_sync, spiir_bank_reset, spiir_bank_destroy, spiir_bank_num_templates,
                       spiir_bank_num_filters, spiir_bank_max_delay, spiir_bank_get_state,
                       spiir_bank_set_state, spiir_kernel_launches, spiir_last_error, spiir_version,

@@ -16,7 +16,7 @@ EXPORTS = ["spiir_bank_create", "spiir_filter", "spiir_filter_host", "spiir_bank
            "spiir_bank_num_templates", "spiir_bank_num_filters", "spiir_bank_max_delay",
            "spiir_bank_get_state", "spiir_bank_set_state", "spiir_bank_destroy", "spiir_last_error",
            "spiir_kernel_launches", "spiir_bank_last_path", "spiir_version", "spiir_layout_probe",
-           "spiir_filter_host_async", "spiir_bank_host_sync", "spiir_filter_peaks"]
+           "spiir_filter_host_async", "spiir_bank_host_sync", "spiir_filter_peaks", "spiir_filter_static"]
 
 
 class SpiirError(RuntimeError):
@@ -60,6 +60,8 @@ def load_library():
     lib.spiir_bank_create.argtypes = [ctypes.POINTER(vp), i32, vp, vp, vp, vp, i32, ctypes.POINTER(SpiirOptions)]
     lib.spiir_filter.restype = ctypes.c_int
     lib.spiir_filter.argtypes = [vp, vp, i64, vp, i64, vp]
+    lib.spiir_filter_static.restype = ctypes.c_int
+    lib.spiir_filter_static.argtypes = [vp, vp, i64, vp, i64, vp]
     lib.spiir_filter_host.restype = ctypes.c_int
     lib.spiir_filter_host.argtypes = [vp, vp, i64, vp, i64]
     lib.spiir_filter_host_async.restype = ctypes.c_int
@@ -152,6 +154,24 @@ def spiir_filter(bank, x, snr, ld: int | None = None, stream=None, n: int | None
         ld = int(snr.stride(0)) if snr.shape[0] > 1 else max(int(snr.shape[1]), n)
     _check(load_library().spiir_filter(bank, ctypes.c_void_p(x.data_ptr()), n, ctypes.c_void_p(snr.data_ptr()),
                                        int(ld), _stream_handle(stream)))
+
+
+def spiir_filter_static(bank, x, snr, ld: int | None = None, stream=None):
+    """``spiir_filter`` through the entry point that allocates nothing (SPIIR_PATH_STREAM banks, n <= 64, <= 8192 warp
+    tiles): the partial sums go to a 4 MiB file-scope device array of the library instead of a cudaMalloc'ed buffer."""
+    import torch
+    if x.dtype != torch.float32 or not x.is_cuda or not x.is_contiguous():
+        raise ValueError("x must be a contiguous CUDA float32 tensor")
+    if snr.dtype != torch.complex64 or not snr.is_cuda or snr.device != x.device:
+        raise ValueError("snr must be a CUDA complex64 tensor on x's device")
+    _check_rows(bank, snr)
+    n = int(x.numel())
+    if ld is None:
+        if snr.dim() != 2 or (snr.shape[1] > 1 and snr.stride(1) != 1) or snr.shape[1] < n:
+            raise ValueError("snr must be [T, >=n] with unit column stride")
+        ld = int(snr.stride(0)) if snr.shape[0] > 1 else max(int(snr.shape[1]), n)
+    _check(load_library().spiir_filter_static(bank, ctypes.c_void_p(x.data_ptr()), n, ctypes.c_void_p(snr.data_ptr()),
+                                              int(ld), _stream_handle(stream)))
 
 
 def spiir_filter_prepared(bank, x, snr, ld: int | None = None, stream=None):

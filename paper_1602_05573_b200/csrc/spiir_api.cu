@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -75,6 +76,34 @@ cudaError_t upload(T** dst, const std::vector<T>& v)
     return e;
 }
 
+}  // namespace
+
+// ---- scratch of the entry point that allocates nothing (spiir_filter_static, see include/spiir.h).
+// File-scope device array of a fixed, modest size: every GPU that loads the library holds these 4 MiB until exit.  In host
+// code the array's name is only a stand-in, not a device address: the address is looked up once per device with
+// cudaGetSymbolAddress (that device current) and handed to the kernels.
+constexpr int64_t kStaticStreamTiles = 8192;       // warp tiles (32 * filters_per_thread filter slots each)
+static __device__ __align__(256) unsigned long long g_static_stream_scratch[kStaticStreamTiles * spiir::kStreamMax];
+
+namespace {
+constexpr int kMaxDevices = 64;
+unsigned long long* g_static_scratch_addr[kMaxDevices] = {nullptr};
+std::mutex g_static_scratch_mutex;
+
+// The device address of g_static_stream_scratch on `device`, which must be the current device.
+int static_scratch_address(int device, unsigned long long** out)
+{
+    if (device < 0 || device >= kMaxDevices) return fail(SPIIR_EINVAL, "device %d beyond the %d the static scratch serves", device, kMaxDevices);
+    std::lock_guard<std::mutex> lock(g_static_scratch_mutex);
+    if (!g_static_scratch_addr[device]) {
+        unsigned long long* ptr = nullptr;
+        CU_TRY(cudaGetSymbolAddress((void**)&ptr, g_static_stream_scratch));
+        if (!ptr) return fail(SPIIR_ECUDA, "cudaGetSymbolAddress returned a null address for the static scratch");
+        g_static_scratch_addr[device] = ptr;
+    }
+    *out = g_static_scratch_addr[device];
+    return SPIIR_OK;
+}
 }  // namespace
 
 struct spiir_bank {
@@ -1055,6 +1084,100 @@ int spiir_bank_set_state(spiir_bank* bk, const float* y_dev, const float* hist_d
     if (hist_dev && bk->D > 0)
         CU_TRY(cudaMemcpyAsync(bk->tape[bk->cur] + bk->pos - bk->D, hist_dev, (size_t)bk->D * sizeof(float),
                                cudaMemcpyDeviceToDevice, st));
+    return SPIIR_OK;
+}
+
+// The entry point that allocates nothing (include/spiir.h): a tiny-chunk call of a SPIIR_PATH_STREAM bank whose per-tile
+// partial sums go to the file-scope device array g_static_stream_scratch instead of a cudaMalloc'ed buffer.  It never
+// reaches cudaMalloc / cudaFree: sizes beyond the array, calls that would grow the tape and stream switches that would
+// create an event are rejected.  The kernels are the ones spiir_filter launches for such a call.
+int spiir_filter_static(spiir_bank* bk, const float* x_dev, int64_t n, float* snr_dev, int64_t ld, void* stream)
+{
+    if (!bk) return fail(SPIIR_EINVAL, "null bank");
+    if (bk->poisoned) return fail(SPIIR_ESTATE, "bank unusable after an earlier failure");
+    if (n < 0 || ld < n) return fail(SPIIR_EINVAL, "need 0 <= n <= ld");
+    if (n == 0) return SPIIR_OK;
+    if (!x_dev || !snr_dev) return fail(SPIIR_EINVAL, "null device pointer");
+    if (bk->opt.path != SPIIR_PATH_STREAM)
+        return fail(SPIIR_EINVAL, "spiir_filter_static serves banks created with SPIIR_PATH_STREAM only");
+    if (n > kStreamMax)
+        return fail(SPIIR_EINVAL, "spiir_filter_static: n = %lld exceeds the %d samples per call of the streaming kernels",
+                    (long long)n, kStreamMax);
+    if (bk->n_tiles > kStaticStreamTiles)
+        return fail(SPIIR_EINVAL, "spiir_filter_static: the bank has %lld warp tiles, the static scratch holds %lld (= %lld filter "
+                    "slots at %d filters per thread); use spiir_filter", (long long)bk->n_tiles, (long long)kStaticStreamTiles,
+                    (long long)(kStaticStreamTiles * kWarp * bk->F), bk->F);
+    cudaStream_t st = (cudaStream_t)stream;
+    DeviceGuard dg(bk->device);
+    CU_TRY(dg.err);
+    if (bk->cap < round_up(bk->D, 4) + n + 16)
+        return fail(SPIIR_EINVAL, "spiir_filter_static: the input tape would have to grow (allocation); use spiir_filter");
+    if (bk->last_stream_valid && bk->last_stream != st && !bk->ev_order)
+        return fail(SPIIR_EINVAL, "spiir_filter_static: the previous call of this bank used another stream and ordering the two "
+                    "would create an event; keep the bank on one stream");
+    int rc = order_after_previous(bk, st);
+    if (rc) return rc;
+    rc = ensure_tape(bk, n, st);              // room is there: at most the compaction copy (cudaMemcpyAsync)
+    if (rc) return rc;
+    float* tape = bk->tape[bk->cur];
+    const int64_t start_al = (bk->pos - bk->D) / 4 * 4;
+    const int w0 = (int)(bk->pos - start_al);
+    if (!stream_applies(bk, w0, n))
+        return fail(SPIIR_EINVAL, "spiir_filter_static: the history of this bank does not fit the streaming kernel's shared memory");
+    unsigned long long* scratch = nullptr;
+    rc = static_scratch_address(bk->device, &scratch);      // cudaGetSymbolAddress, once per device
+    if (rc) return rc;
+    NvtxRange range("spiir_filter_static: tiny-chunk streaming path, static scratch");
+    const void* fn = select_stream_kernel(bk->F, bk->NC);
+    if (!bk->stream_configured) {
+        CU_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bk->smem_optin));
+        bk->stream_configured = true;
+    }
+    const int kStreamWarps = stream_warps(bk->F);
+    const size_t smem = stream_smem_bytes(bk->F, bk->NC, w0 + n, nullptr);
+    if (bk->stream_occ_smem != smem) {
+        int occ = 0;
+        CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kWarp * kStreamWarps, smem));
+        if (occ < 1) return fail(SPIIR_ECUDA, "streaming kernel does not fit on an SM (smem %zu)", smem);
+        bk->stream_occ = occ;
+        bk->stream_occ_smem = smem;
+    }
+    StreamParams p{};
+    p.coef = bk->coef; p.y = bk->y;
+    p.xwin = tape + start_al; p.w0 = w0; p.n = (int32_t)n; p.n_tiles = bk->n_tiles; p.scratch = scratch;
+    p.xnew = x_dev; p.append = tape + bk->pos;
+    const int64_t ctas = std::min<int64_t>((bk->n_tiles + kStreamWarps - 1) / kStreamWarps, (int64_t)bk->n_sm * bk->stream_occ);
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)ctas, 1, 1);
+        cfg.blockDim = dim3(kWarp * kStreamWarps, 1, 1);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        void* args[] = {(void*)&p};
+        CU_TRY(cudaLaunchKernelExC(&cfg, fn, args));
+    }
+    {
+        const int64_t total = bk->T * n;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)((total + 255) / 256), 1, 1);
+        cfg.blockDim = dim3(256, 1, 1);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = st;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        CU_TRY(cudaLaunchKernelEx(&cfg, spiir_stream_combine_kernel, (const u64*)scratch, (const int64_t*)bk->tile_begin,
+                                  (int32_t)bk->T, (int32_t)n, snr_dev, ld, (u64*)nullptr));
+    }
+    g_launches.fetch_add(2, std::memory_order_relaxed);
+    rc = SPIIR_OK;
+    if (cudaGetLastError() != cudaSuccess) { bk->poisoned = true; return fail(SPIIR_ECUDA, "spiir_filter_static: launch failed"); }
+    bk->last_path = SPIIR_PATH_STREAM;
+    bk->pos += n;
     return SPIIR_OK;
 }
 
