@@ -78,9 +78,10 @@ typedef struct spiir_options {
                                    filters_per_thread 4, 8 or 16 there */
     int32_t window_copies;      /* 0 = choose; else 1, 2 or 4 shifted copies of the input window in shared memory
                                    (= floats per shared-memory load); falls back if they do not fit */
-    int32_t small_templates;    /* templates of <= 128 filters sharing warp tiles (sub-warp segments):
-                                   0 = choose, 1 = on (forces the (8,16) blocking), 2 = off.  Not used with
-                                   SPIIR_PATH_STREAM. */
+    int32_t small_templates;    /* templates of <= 16 x filters_per_thread filters sharing warp tiles (sub-warp segments of 4,
+                                   8 or 16 lanes): 0 = choose, 1 = on, 2 = off.  Shared tiles exist
+                                   for the blockings (8,16), (4,16) and (2,32); the cheapest for the bank is taken unless
+                                   filters_per_thread / warps_per_cta name one.  Not used with SPIIR_PATH_STREAM. */
     int32_t scan_launches;      /* kernel launches per call of the two low-latency paths.  0 = choose: SPIIR_PATH_SCAN takes
                                    one cooperative launch when every CTA of the items x segments grid is resident (else
                                    three), SPIIR_PATH_STREAM a tile kernel + a combine kernel chained by programmatic

@@ -254,16 +254,18 @@ int ensure_tape(spiir_bank* bk, int64_t n, cudaStream_t st)
 // a 16 384-sample chunk behind a 16 383-sample history allows only one).
 const void* select_kernel(int F, int W, int NC, bool g, bool peak = false, bool seg = false)
 {
-    if (seg) {      // shared tiles of small templates: one blocking, F = 8 / 16 warps (32-filter templates on 4 lanes)
-        if (F != 8 || W != 16) return nullptr;
-#define SPIIR_SEG(P_)                                                                           \
-        if (g) return (const void*)spiir_filter_kernel<8, 16, 1, true, 1, P_, true>;            \
-        if (NC == 4) return (const void*)spiir_filter_kernel<8, 16, 4, false, 1, P_, true>;     \
-        if (NC == 2) return (const void*)spiir_filter_kernel<8, 16, 2, false, 1, P_, true>;     \
-        return (const void*)spiir_filter_kernel<8, 16, 1, false, 1, P_, true>;
-        if (peak) { SPIIR_SEG(true) }
-        SPIIR_SEG(false)
+    if (seg) {      // shared tiles of small templates: F = 8 / 16 warps, and F = 4 / 16 and F = 2 / 32 warps for tiny ones
+#define SPIIR_SEG(F_, W_, P_)                                                                       \
+        if (F == F_ && W == W_) {                                                                   \
+            if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true, 1, P_, true>;           \
+            if (NC == 4) return (const void*)spiir_filter_kernel<F_, W_, 4, false, 1, P_, true>;    \
+            if (NC == 2) return (const void*)spiir_filter_kernel<F_, W_, 2, false, 1, P_, true>;    \
+            return (const void*)spiir_filter_kernel<F_, W_, 1, false, 1, P_, true>;                 \
+        }
+        if (peak) { SPIIR_SEG(8, 16, true) SPIIR_SEG(4, 16, true) SPIIR_SEG(2, 32, true) }
+        else { SPIIR_SEG(8, 16, false) SPIIR_SEG(4, 16, false) SPIIR_SEG(2, 32, false) }
 #undef SPIIR_SEG
+        return nullptr;
     }
 #define SPIIR_VARIANT_P(F_, W_, M_, P_)                                                        \
         if (g) return (const void*)spiir_filter_kernel<F_, W_, 1, true, M_, P_>;               \
@@ -632,9 +634,11 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
 
 // Relative cost per padded filter slot of the compiled blockings, measured on padding-free banks (cfg3 for F >= 8,
 // banks of 32- to 128-filter templates below): F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 ~ 42 %,
-// F = 2 ~ 29 %, F = 1 (one warp per template) ~ 21 % of FP32 peak; shared tiles (F = 8) ~ 34.5 %.
-double slot_cost(int F) { return F == 16 ? 1.0 : (F == 8 ? 1.05 : (F == 4 ? 1.3 : (F == 2 ? 1.85 : 2.6))); }
-constexpr double kSharedTileCost = 1.57;
+// F = 2 ~ 29 %, F = 1 (one warp per template) ~ 21 % of FP32 peak; shared tiles 43 % (F = 8), 37.5 % (F = 4),
+// 27 % (F = 2).
+double slot_cost(int F) { return F == 16 ? 1.0 : (F == 8 ? 1.06 : (F == 4 ? 1.37 : (F == 2 ? 1.9 : 2.6))); }
+// shared tiles of small templates (padding-free banks of 32- to 128-filter templates: 43 % of peak at F = 8)
+double shared_tile_cost(int F) { return F == 8 ? 1.31 : (F == 4 ? 1.5 : 2.05); }
 
 int choose_F(int32_t T, const int64_t* off, int requested, double* cost_out = nullptr)
 {
@@ -739,26 +743,36 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
     bool segmented = false;
     // Small templates (<= 128 filters) can share warp tiles (PAPER.md:L333-L335 size-aware mapping):
     // blocking F = 8 / 16 warps.  Taken when asked for, or by itself when its estimated cost is lower.
-    if (!stream && o.small_templates != 2 && (o.filters_per_thread == 0 || o.filters_per_thread == 8) &&
-        (o.warps_per_cta == 0 || o.warps_per_cta == 16)) {
-        double packed = 0;
-        bool any_small = false;
-        for (int32_t t = 0; t < T; ++t) {
-            const int64_t Kt = off[t + 1] - off[t];
-            const int w = segment_lanes(Kt, 8, true);
-            any_small |= (w < kWarp);
-            packed += w < kWarp ? kSharedTileCost * (double)(w * 8) : slot_cost(8) * (double)((Kt + 255) / 256 * 256);
-        }
-        if (any_small && (o.small_templates == 1 || packed < plain_cost)) {
-            F = 8; W = 16; segmented = true;
-        }
-    }
     // A bank that fits one CTA at one filter per lane (<= 32 warps x 32 lanes) is bound by latency, not by issue slots:
     // one filter per thread (PAPER.md:L335 one warp per small template) spreads it over the most warps.
-    if (!stream && !segmented && !o.filters_per_thread && (o.warps_per_cta == 0 || o.warps_per_cta == 32)) {
+    bool tiny = false;
+    if (!stream && !o.filters_per_thread && o.small_templates != 1 && (o.warps_per_cta == 0 || o.warps_per_cta == 32)) {
         int64_t slots1 = 0;
         for (int32_t t = 0; t < T; ++t) slots1 += round_up(off[t + 1] - off[t], kWarp);
-        if (slots1 <= 32 * kWarp) { F = 1; W = 32; }
+        if (slots1 <= 32 * kWarp) { F = 1; W = 32; tiny = true; }
+    }
+    if (!stream && !tiny && o.small_templates != 2) {
+        double best_packed = 0;
+        int best_F = 0;
+        bool any_small = false;
+        for (int Fs : {8, 4, 2}) {
+            const int Ws = default_warps(Fs);
+            if ((o.filters_per_thread && o.filters_per_thread != Fs) || (o.warps_per_cta && o.warps_per_cta != Ws)) continue;
+            double packed = 0;
+            bool small = false;
+            const int64_t per = 32LL * Fs;
+            for (int32_t t = 0; t < T; ++t) {
+                const int64_t Kt = off[t + 1] - off[t];
+                const int w = segment_lanes(Kt, Fs, true);
+                small |= (w < kWarp);
+                packed += w < kWarp ? shared_tile_cost(Fs) * (double)(w * Fs) : slot_cost(Fs) * (double)((Kt + per - 1) / per * per);
+            }
+            if (small && (!best_F || packed < best_packed)) { best_packed = packed; best_F = Fs; }
+            any_small |= small;
+        }
+        if (any_small && best_F && (o.small_templates == 1 || best_packed < plain_cost)) {
+            F = best_F; W = default_warps(best_F); segmented = true;
+        }
     }
     // The (filters_per_thread, warps_per_cta) pair must be one a compiled kernel serves: checked here, not at the first
     // spiir_filter.  When only one of the two was requested the other follows it.
@@ -780,7 +794,7 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
             return fail(SPIIR_EINVAL, "unsupported blocking: filters_per_thread %d with warps_per_cta %d", F, W);
     }
     if (segmented && !select_kernel(F, W, 1, false, false, true))
-        return fail(SPIIR_EINVAL, "shared tiles of small templates need the (8, 16) blocking");
+        return fail(SPIIR_EINVAL, "shared tiles of small templates need the (8, 16), (4, 16) or (2, 32) blocking");
 
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0)

@@ -489,6 +489,8 @@ __device__ __forceinline__ void filter_body(const FilterParams& p, const int seg
                     }
                 }
             } else {
+                // a round made of shared tiles only has nothing to hand over between warps: no CTA-wide barrier in its loop
+                const bool round_bar = !SEG || __syncthreads_or(active && seg_w == 0);
                 int buf = 0;
                 for (int64_t st = 0; st < nseg; st += TS, buf ^= 1) {
                     const int ns = (int)min((int64_t)TS, nseg - st);
@@ -511,7 +513,7 @@ __device__ __forceinline__ void filter_body(const FilterParams& p, const int seg
                             }
                         }
                     }
-                    if (sums) {
+                    if (sums && round_bar) {
                         __syncthreads();
                         if (active && !(SEG && seg_w))
                             cross_warp_store<TS, PEAK>(part64 + (size_t)buf * W * TS, ww, warp, lane, ns, (!PEAK || out_row) ? out_row + st : nullptr, accumulate, peak, idx_row + st);
@@ -526,7 +528,8 @@ __device__ __forceinline__ void filter_body(const FilterParams& p, const int seg
                     *reinterpret_cast<u64*>(yo + 2 * s) = Y[f];
                 }
             }
-            if (sums && !async) __syncthreads();      // part rows are rewritten in the next round
+            if (sums && !async) __syncthreads();      // part rows are rewritten in the next round (kept for shared tiles too:
+                                                      // once per round, and the next round's __syncthreads_or needs all warps)
         }
     }
 }

@@ -129,6 +129,58 @@ inline void deal_groups(const int32_t* d, const std::vector<int64_t>& order, int
     }
 }
 
+// A small template in a shared tile: its K_t filters go into `rows` register slots of w lanes each.  The w lanes of a row
+// are read by the same load instruction (they sit inside one phase, or make up one, for w <= 32 / NC), so a row should hold
+// distinct keys: fullest key classes first, every filter into the row that has the fewest of its key, then the emptiest,
+// then the lowest; all rows but the last are full, so that the padding lands at the end.  Delay-sorted filters are dealt
+// badly by position alone: K_t uniform delays over D samples are D / K_t apart, which is a multiple of the bank-group
+// period as often as not.  The arrangement is a function of the template's own filters only (and of the bank-wide NC).
+inline void deal_rows(const int32_t* d, const std::vector<int64_t>& order, int rows, int w, int NC,
+                      std::vector<std::vector<int64_t>>& out)
+{
+    const int P = kWarp / NC;
+    const int U = std::min(w, P);            // lanes dealt together: a whole phase, or the template's part of one
+    const int per_row = w / U, units = rows * per_row;
+    std::vector<std::vector<int64_t>> bucket(P), unit(units);
+    for (int64_t k : order) bucket[conflict_key(d[k], NC, P)].push_back(k);
+    std::vector<int> rorder(P);
+    std::iota(rorder.begin(), rorder.end(), 0);
+    std::stable_sort(rorder.begin(), rorder.end(), [&](int a, int b) { return bucket[a].size() > bucket[b].size(); });
+    std::vector<int> cap(units, 0), fill(units, 0), mult((size_t)units * P, 0), deg(units, 0);
+    {
+        int64_t left = (int64_t)order.size();
+        for (int g = 0; g < units; ++g) { cap[g] = (int)std::min<int64_t>(U, left); left -= cap[g]; }
+    }
+    // A whole phase costs as many wavefronts as its most frequent key (its degree): a filter that has to double up goes where
+    // the degree does not grow (a phase that already holds a double), then where its key is rarest, then to the emptiest.
+    // A template that fills only part of a phase (w < P) shares it with neighbours it does not know: there the doubles are
+    // spread evenly instead (rarest key, then emptiest), which measures better than concentrating them.
+    const bool whole = (w >= P);
+    for (int r : rorder)
+        for (int64_t k : bucket[r]) {
+            int best = -1, best_grow = 0;
+            for (int g = 0; g < units; ++g) {
+                if (fill[g] >= cap[g]) continue;
+                const int m = mult[(size_t)g * P + r];
+                const int grow = whole ? std::max(deg[g], m + 1) - deg[g] : 0;
+                if (best < 0 || grow < best_grow || (grow == best_grow && (m < mult[(size_t)best * P + r] ||
+                    (m == mult[(size_t)best * P + r] && fill[g] < fill[best])))) {
+                    best = g;
+                    best_grow = grow;
+                }
+            }
+            unit[best].push_back(k);
+            ++fill[best];
+            deg[best] = std::max(deg[best], ++mult[(size_t)best * P + r]);
+        }
+    // lanes of a unit in delay order (ties by caller index): any order is equally conflict-free; a row = per_row units
+    out.assign(rows, {});
+    for (int g = 0; g < units; ++g) {
+        std::sort(unit[g].begin(), unit[g].end(), [&](int64_t x, int64_t y) { return d[x] != d[y] ? d[x] < d[y] : x < y; });
+        out[g / per_row].insert(out[g / per_row].end(), unit[g].begin(), unit[g].end());
+    }
+}
+
 // Lanes a small template occupies in a shared ("segmented") warp tile: the smallest of 4, 8, 16 whose lanes x F
 // register slots hold its K_t filters; 32 = a template that gets warp tiles of its own (PAPER.md:L333-L335 maps
 // templates of <= 32 filters to one warp; here several of them share one warp so that every lane still runs F filters).
@@ -200,23 +252,26 @@ inline HostLayout build_layout(int32_t T, const int64_t* off, const float* a1, c
         std::iota(order.begin(), order.end(), k0);
         std::stable_sort(order.begin(), order.end(), [&](int64_t x, int64_t y) { return d[x] < d[y]; });
         if (seg_w[t] < kWarp) {
-            // small template: lanes [seg * w, seg * w + w) of a shared tile, filter i (delay order) -> lane i % w, slot i / w
+            // small template: lanes [seg * w, seg * w + w) of a shared tile; its filters dealt to the F rows of those lanes
             const int w = seg_w[t];
             const int64_t tile = L.tile_begin[t];
-            for (int64_t i = 0; i < (int64_t)w * F; ++i) {
-                const int64_t s = (tile * F + i / w) * kWarp + (int64_t)seg_idx[t] * w + i % w;
-                if (i < Kt) {
-                    const int64_t k = order[(size_t)i];
-                    L.ar[s] = a1[2 * k];
-                    L.ai[s] = a1[2 * k + 1];
-                    L.b[2 * s] = b0[2 * k];
-                    L.b[2 * s + 1] = b0[2 * k + 1];
-                    L.dly[s] = d[k];
-                    L.slot_of_filter[k] = s;
-                } else {
-                    L.dly[s] = d[order[0]];           // null filter: any valid window position
+            deal_rows(d, order, F, w, NC, groups);
+            for (int g = 0; g < F; ++g)
+                for (int l = 0; l < w; ++l) {
+                    const int64_t s = (tile * F + g) * kWarp + (int64_t)seg_idx[t] * w + l;
+                    if (l < (int)groups[g].size()) {
+                        const int64_t k = groups[g][(size_t)l];
+                        L.ar[s] = a1[2 * k];
+                        L.ai[s] = a1[2 * k + 1];
+                        L.b[2 * s] = b0[2 * k];
+                        L.b[2 * s + 1] = b0[2 * k + 1];
+                        L.dly[s] = d[k];
+                        L.slot_of_filter[k] = s;
+                    } else {
+                        // null filter: the address of a real lane of the row (broadcast), else any valid window position
+                        L.dly[s] = groups[g].empty() ? d[order[0]] : d[groups[g][0]];
+                    }
                 }
-            }
             continue;
         }
         const int64_t nt = (Kt + per_tile - 1) / per_tile;

@@ -194,20 +194,23 @@ def test_bank_of_very_small_templates(env):
     check(run_gpu(env, inp, chunks=[64] * 14 + [4], path=3, rows=rows), ref)
 
 
-def test_small_templates_share_warp_tiles(env):
+@pytest.mark.parametrize("F", [0, 8, 4, 2])
+def test_small_templates_share_warp_tiles(env, F):
     # sub-warp segments: 4-, 8- and 16-lane segments, partially filled tiles, size
-    # classes changing along the bank, and large templates in between
+    # classes changing along the bank, and large templates in between; shared-tile blockings (8,16), (4,16), (2,32)
     counts = [32, 17, 8, 1, 32, 30, 2, 25, 64, 33, 60, 128, 100, 65, 700, 12, 12, 12, 128, 129, 5] * 6
     inp = spiir_inputs.make_random_bank(62, counts, 1100, d_max=400)
     ref = env[1].run_inputs(inp)
     for path in (1, 2):
-        check(run_gpu(env, inp, chunks=[500, 7, 593], path=path, small=1), ref)
-    a = run_gpu(env, inp, chunks=[500, 600], path=1, small=1)
-    assert np.array_equal(a.view(np.float32), run_gpu(env, inp, chunks=[500, 600], path=1, small=1).view(np.float32))
+        check(run_gpu(env, inp, chunks=[500, 7, 593], path=path, small=1, F=F), ref)
+    a = run_gpu(env, inp, chunks=[500, 600], path=1, small=1, F=F)
+    assert np.array_equal(a.view(np.float32), run_gpu(env, inp, chunks=[500, 600], path=1, small=1, F=F).view(np.float32))
     # a template's sums do not depend on which segment of which tile it landed in
     perm = np.random.default_rng(1).permutation(len(counts))
-    b = run_gpu(env, inp.select_templates(perm), chunks=[500, 600], path=1, small=1)
+    b = run_gpu(env, inp.select_templates(perm), chunks=[500, 600], path=1, small=1, F=F)
     assert np.array_equal(b.view(np.float32), a[perm].view(np.float32))
+    if F:
+        return
     # chosen by itself for a bank of tiny templates, and the host entry works on it
     tiny = spiir_inputs.make_random_bank(63, [32, 20, 31] * 100, 600, d_max=300)
     check(run_gpu(env, tiny, chunks=[600]), env[1].run_inputs(tiny))
