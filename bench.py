@@ -10,7 +10,7 @@ timed region starts (`value`); `e2e` repeats the measurement through spiir_filte
 (H2D of every chunk and D2H of every SNR block inside the timed region).  Prints ONE JSON line.
 
 The default run (N = 1, --config 3) also times every other config of BASELINE.json in short legs and reports them
-under `per_config` (cfg0, cfg1 one-shot and 16 x 4096, cfg2, cfg4: filter-samples/s, roofline fraction, per-call
+under `per_config` (cfg0, cfg1 one-shot and 16 x 4096, cfg2, cfg4, two banks of small templates: filter-samples/s, roofline fraction, per-call
 p50/p99, path taken, clocks of that leg); --no-per-config skips them.
 
 N > 1 (torchrun, one rank per GPU): templates are independent, so every rank filters
@@ -191,11 +191,11 @@ def setup(args):
     return torch, dist, pkg, world, rank, dev_index, red_dev, oversubscribed
 
 
-def measure(ctx, args, cfg, steps, warmup, *, chunk=None, e2e=False, label=None):
+def measure(ctx, args, cfg, steps, warmup, *, chunk=None, e2e=False, label=None, inp=None):
     """Time `steps` steps of configs[cfg] on this rank's GPU (a step = the config's whole streaming run; chunk=0: one call
     over the whole series).  -> dict with value, ms_per_step, roofline, latency, clocks, launches, path (+ e2e)."""
     torch, dist, pkg, world, rank, dev_index, red_dev, oversubscribed = ctx
-    inp = spiir_inputs.make_config(cfg)
+    inp = spiir_inputs.make_config(cfg) if inp is None else inp        # inp given: a workload outside BASELINE.json:configs
     shard_info = None
     if args.shard and world > 1:
         # ONE bank split over the ranks by template (DESIGN.md section 9; SURVEY.md section 8(e)): longest-processing-time
@@ -401,8 +401,16 @@ def run_ours(args):
         per = {}
         legs = [("cfg0", 0, None, 200), ("cfg1_oneshot", 1, 0, 20), ("cfg1_chunked", 1, None, 10), ("cfg2", 2, None, 5),
                 ("cfg4", 4, None, 2)]
+        # + banks of small templates: 32 768 templates of 32 filters and 65 536
+        #   of 8, cfg1's distributions, delays up to 2047, 4 calls of 4096 samples
+        small = {"small_templates_32": (32, 32768), "small_templates_8": (8, 65536)}
+        legs += [(name, -1, None, 5) for name in small]
         for name, cfg, chunk, steps in legs:
-            r = measure(ctx, args, cfg, steps, 3, chunk=chunk)
+            override = None
+            if name in small:
+                kt, nt = small[name]
+                override = spiir_inputs.make_random_bank(7 + kt, [kt] * nt, 16384, d_max=2047, chunk=4096, name=name)
+            r = measure(ctx, args, cfg, steps, 3, chunk=chunk, inp=override)
             r.pop("_inp")
             rf = r["roofline"]
             per[name] = {"workload": r["workload"], "value": r["value"], "unit": UNIT, "steps": steps, "ms_per_step": r["ms_per_step"],

@@ -86,7 +86,7 @@ def test_bench_default_run_reports_every_config():
     check_line(d)
     assert d["e2e"].get("last_chunk_bitwise_equal_to_device_run") is True
     per = d["per_config"]
-    assert set(per) == {"cfg0", "cfg1_oneshot", "cfg1_chunked", "cfg2", "cfg4"}
+    assert set(per) == {"cfg0", "cfg1_oneshot", "cfg1_chunked", "cfg2", "cfg4", "small_templates_32", "small_templates_8"}
     for name, leg in per.items():
         assert leg["value"] > 0 and leg["bound"] in ("alu", "hbm") and 0 < leg["frac"] < 1.2, name
         assert leg["p50_us"] > 0 and leg["p99_us"] >= leg["p50_us"] and "reasons" in leg["clocks"], name
