@@ -401,9 +401,9 @@ def run_ours(args):
         per = {}
         legs = [("cfg0", 0, None, 200), ("cfg1_oneshot", 1, 0, 20), ("cfg1_chunked", 1, None, 10), ("cfg2", 2, None, 5),
                 ("cfg4", 4, None, 2)]
-        # + banks of small templates: 32 768 templates of 32 filters and 65 536
-        #   of 8, cfg1's distributions, delays up to 2047, 4 calls of 4096 samples
-        small = {"small_templates_32": (32, 32768), "small_templates_8": (8, 65536)}
+        # + banks of small templates: 37 888 templates of 32 filters and 75 776
+        #   of 8 (two full waves of CTA items on 148 SMs each), cfg1's distributions, delays up to 2047, 4 calls of 4096 samples
+        small = {"small_templates_32": (32, 37888), "small_templates_8": (8, 75776)}
         legs += [(name, -1, None, 5) for name in small]
         for name, cfg, chunk, steps in legs:
             override = None

@@ -632,13 +632,18 @@ int run_chunk(spiir_bank* bk, const float* xwin, int w0, int64_t n, float* snr, 
     return SPIIR_OK;
 }
 
-// Relative cost per padded filter slot of the compiled blockings, measured on padding-free banks (cfg3 for F >= 8,
-// banks of 32- to 128-filter templates below): F = 16 / 8 warps 54.3 %, F = 8 / 16 warps 51.7 %, F = 4 ~ 42 %,
-// F = 2 ~ 29 %, F = 1 (one warp per template) ~ 21 % of FP32 peak; shared tiles 43 % (F = 8), 37.5 % (F = 4),
-// 27 % (F = 2).
-double slot_cost(int F) { return F == 16 ? 1.0 : (F == 8 ? 1.06 : (F == 4 ? 1.37 : (F == 2 ? 1.9 : 2.6))); }
-// shared tiles of small templates (padding-free banks of 32- to 128-filter templates: 43 % of peak at F = 8)
-double shared_tile_cost(int F) { return F == 8 ? 1.31 : (F == 4 ? 1.5 : 2.05); }
+// Relative cost per padded filter slot of the compiled blockings, measured on padding-free banks that fill whole waves of CTA
+// items (cfg3 for F = 16; banks of 4- to 256-filter templates below; product build): plain tiles F = 16 / 8 warps 56.2 %,
+// F = 8 / 16 warps 53.7 %, F = 4 / 16 warps 47.5 %, F = 2 / 32 warps 36 %, F = 1 (one warp per template) ~ 21 %
+// of FP32 peak; shared tiles F = 8: 50.5 % for segments of 8 or 16 lanes, 42.8 % for full 4-lane
+// segments (they share a load phase with a neighbour), F = 4: 42.4 / 45.6 / 43.5 % for 4 / 8 / 16 lanes, F = 2: 28 - 34 %.
+double slot_cost(int F) { return F == 16 ? 1.0 : (F == 8 ? 1.05 : (F == 4 ? 1.18 : (F == 2 ? 1.56 : 2.6))); }
+double shared_tile_cost(int F, int w, double fill)
+{
+    if (F == 8) return w == 4 ? 1.13 + 0.18 * fill * fill : 1.11;      // padding lanes broadcast: fewer conflicts when not full
+    if (F == 4) return w == 4 ? 1.33 : (w == 8 ? 1.23 : 1.29);
+    return w == 4 ? 2.0 : (w == 8 ? 1.8 : 1.66);
+}
 
 int choose_F(int32_t T, const int64_t* off, int requested, double* cost_out = nullptr)
 {
@@ -765,7 +770,8 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
                 const int64_t Kt = off[t + 1] - off[t];
                 const int w = segment_lanes(Kt, Fs, true);
                 small |= (w < kWarp);
-                packed += w < kWarp ? shared_tile_cost(Fs) * (double)(w * Fs) : slot_cost(Fs) * (double)((Kt + per - 1) / per * per);
+                packed += w < kWarp ? shared_tile_cost(Fs, w, (double)Kt / (double)(w * Fs)) * (double)(w * Fs)
+                                    : slot_cost(Fs) * (double)((Kt + per - 1) / per * per);
             }
             if (small && (!best_F || packed < best_packed)) { best_packed = packed; best_F = Fs; }
             any_small |= small;
@@ -832,8 +838,9 @@ int spiir_bank_create(spiir_bank** out, int32_t T, const int64_t* off, const flo
                 continue;
             }
 
-            // F = 16 keeps 2 copies: its LDS.128 variant needs all 255 registers and measures 8 % slower (cfg2: 43.2 -> 46.6 %)
-            if (nc == 4 && bk->F == 16) continue;
+            // F >= 8 keeps 2 copies: the LDS.128 variants are short of registers (F = 16: all 255, 8 % slower on cfg2; F = 8: 128
+            // with a spill, 1 - 3 % slower on banks of 64- to 256-filter templates)
+            if (nc == 4 && bk->F >= 8) continue;
             if ((hist + kMinSub) * 4 * nc <= room) { bk->NC = nc; break; }
         }
         if (o.window_copies == 1 || o.window_copies == 2 || o.window_copies == 4)
