@@ -113,6 +113,47 @@ def test_small_templates_pack_into_shared_tiles(pkg):
     assert tile[inp.offsets[8]] != tile[inp.offsets[7]]
 
 
+def test_shared_tile_segments_are_dealt_by_conflict_key(pkg):
+    """Inside a segment the filters of one register slot are read by one load phase: they are dealt by conflict key, not by
+    position in delay order (uniform delays D / K_t apart are a multiple of the bank-group period as often as not)."""
+    def brute_degree(offsets, delays, slots, F, NC):
+        """mean over load phases (32 / NC consecutive lanes of one register slot) of the largest key multiplicity"""
+        P = 32 // NC
+        key = (delays.astype(np.int64) + NC - 1) // NC % P
+        phase = slots // 32 * NC + slots % 32 // P                     # (tile, slot) row x phase within the row
+        deg = []
+        for ph in np.unique(phase):
+            deg.append(np.bincount(key[phase == ph], minlength=P).max())
+        return float(np.mean(deg))
+    for kt, limit in ((64, 1.7), (128, 1.55), (100, 1.55)):
+        inp = spiir_inputs.make_random_bank(5, [kt] * 256, 8, d_max=2047)
+        slots, st = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, 4, True)
+        assert st["segmented"] == 1
+        assert st["avg_conflict_degree"] == pytest.approx(brute_degree(inp.offsets, inp.delays, slots, 8, 4), abs=1e-9)
+        assert st["avg_conflict_degree"] <= limit, (kt, st["avg_conflict_degree"])      # by position in delay order: 1.9
+    # regular spacing, the worst case of dealing by position: 64 filters 32 samples apart all have the same key
+    off = np.arange(0, 65 * 64, 64)
+    d = np.tile(np.arange(64, dtype=np.int32) * 32, 64)
+    slots, st = pkg.spiir_layout_probe(off, d, 8, 16, 4, True)
+    assert st["avg_conflict_degree"] == 8.0                            # nothing to deal: one key class
+    d = np.tile(np.arange(64, dtype=np.int32) * 33, 64)                # keys 0..7 cyclically: perfect phases exist
+    slots, st = pkg.spiir_layout_probe(off, d, 8, 16, 4, True)
+    assert st["avg_conflict_degree"] <= 1.15
+    # the arrangement of a template does not depend on where it sits in the bank
+    inp = spiir_inputs.make_random_bank(6, [64, 20, 64, 33, 64], 8, d_max=900)
+    a, _ = pkg.spiir_layout_probe(inp.offsets, inp.delays, 8, 16, 4, True)
+    perm = np.array([2, 3, 4, 0, 1])
+    inp2 = inp.select_templates(perm)
+    b, _ = pkg.spiir_layout_probe(inp2.offsets, inp2.delays, 8, 16, 4, True)
+    F = 8
+    for new_t, old_t in enumerate(perm):
+        sa = a[inp.offsets[old_t]:inp.offsets[old_t + 1]]
+        sb = b[inp2.offsets[new_t]:inp2.offsets[new_t + 1]]
+        w = next(w for w in (4, 8, 16, 32) if w * F >= sa.size)
+        # same register slot and same lane within the segment for every filter
+        assert np.array_equal(sa // 32 % F, sb // 32 % F) and np.array_equal(sa % 32 % w, sb % 32 % w)
+
+
 def test_probe_validates_arguments(pkg):
     with pytest.raises(pkg.SpiirError):
         pkg.spiir_layout_probe(np.array([0, 2]), np.array([0, -1], np.int32))
